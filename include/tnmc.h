@@ -1,0 +1,191 @@
+/* tnmc.h -- C ABI of the B200-native BatchTNMC hot path (arXiv 2509.19006).
+ *
+ * Citations "PAPER.md:NN" refer to /root/reference/PAPER.md; "DESIGN.md Gn / P-C2 / R" are the
+ * readings of the paper listed in DESIGN.md.
+ *
+ * What the library computes, per disorder realisation d of the 2D +-J Ising model on an open
+ * L x L lattice (Eq. 1):
+ *   tnmc_build_envs  the boundary-MPS "cache" of create_cache_ising: the row
+ *                    MPOs of Eq. 7-8 applied bottom-to-top to the
+ *                    bottom-row MPS, each product compressed to bond
+ *                    dimension chi (multiply/compress, PAPER.md:97 Fig. 2, :147, :186-187;
+ *                    reading P-C2), and log Z (Eq. 6);
+ *   tnmc_sample      SamplerIsing.sample/_sample_row: row-by-row ancestral
+ *                    sampling with the right-environment sweep and the left
+ *                    sampling sweep (Eq. 5), returning bit-packed
+ *                    configurations and log q(s) (Eq. 9);
+ *   tnmc_energy      Eq. 1, exact integer arithmetic;
+ *   tnmc_metropolis  the independence Metropolis-Hastings acceptance of Eq. 10.
+ *
+ * Conventions
+ *   rows r = 0..L-1 top to bottom, columns c = 0..L-1 left to right, raster order
+ *   site = r*L + c; spin index a in {0,1} <-> s = 2a-1.
+ *   Jr[d][r][c] couples (r,c)-(r,c+1) (the paper's J_mat[r,c,2]), must be 0 at
+ *   c = L-1; Jd[d][r][c] couples (r,c)-(r+1,c) (J_mat[r,c,3]), must be 0 at r = L-1.
+ *   cfg_bits: uint32 (dis_count, n_samples, L, W) with W = ceil(L/32); bit (c % 32) of word
+ *   c/32 of row r is 1 iff s(r,c) = +1; unused high bits are 0.
+ *   Random numbers (reading R): Philox4x32-10, key = (seed & 0xffffffff, seed >> 32),
+ *   counter = (site, sample index, disorder index, tag), tag 0 = spin draws, tag 1 = Metropolis
+ *   draws (site word 0, sample word = step index); u = ((x0 << 21) | (x1 >> 11)) * 2^-53;
+ *   a spin is +1 iff u < p.  "disorder index" is first_disorder + d, "sample index" is
+ *   sample_offset + n, so results do not depend on how calls are chunked.
+ *
+ * Memory and ownership
+ *   Every pointer marked [dev] is a device pointer owned by the caller (e.g. torch tensors);
+ *   [host] is a host pointer.  The context owns only a few hundred bytes of host metadata; all
+ *   device storage it uses lives inside the caller-provided workspace (size from
+ *   tnmc_workspace_bytes), which must stay alive and untouched until tnmc_destroy.  No entry
+ *   point allocates device memory.  Kernels are enqueued on the stream given to tnmc_create and
+ *   the calls return before completion; outputs are valid after the caller synchronises that
+ *   stream.  Only tnmc_get_flags / tnmc_get_env_row / tnmc_run_host synchronise.
+ *
+ * Errors
+ *   Every call returns a tnmc_status; nothing throws across the ABI.  Argument errors are
+ *   detected synchronously and leave the context unchanged; tnmc_last_error gives a message.
+ *   Numeric faults inside kernels (rho == 0, non-finite values, non-positive sum for log Z,
+ *   Jacobi sweep limit) are counted on the device and read with tnmc_get_flags.
+ *   There is no CPU fallback anywhere: without a CUDA device every compute call fails with
+ *   TNMC_ECUDA.
+ */
+#ifndef TNMC_H_
+#define TNMC_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tnmc_ctx tnmc_ctx; /* opaque, library-owned host object */
+
+typedef enum {
+    TNMC_OK = 0,
+    TNMC_EINVAL = 1,   /* bad argument */
+    TNMC_ENOMEM = 2,   /* workspace too small */
+    TNMC_ECUDA = 3,    /* CUDA runtime error (message in tnmc_last_error) */
+    TNMC_ESTATE = 4,   /* call order: e.g. tnmc_sample before tnmc_build_envs */
+    TNMC_ENUMERIC = 5
+} tnmc_status;
+
+typedef enum {
+    TNMC_F64 = 0 /* FP64 storage and arithmetic (the only precision in this round) */
+} tnmc_prec;
+
+/* indices into the array returned by tnmc_get_flags */
+enum {
+    TNMC_FLAG_RHO_ZERO = 0,      /* a conditional weight rho_a was exactly 0 (reading G10) */
+    TNMC_FLAG_NONFINITE = 1,     /* a non-finite intermediate was seen */
+    TNMC_FLAG_LOGZ_NONPOS = 2,   /* sum_sigma Psi_0(sigma) <= 0 in the log Z read-out */
+    TNMC_FLAG_NEAR_THRESHOLD = 3,/* draws with |u - p| < 1e-9 (north_star parity clause) */
+    TNMC_FLAG_JACOBI_LIMIT = 4,  /* a site SVD hit the sweep limit before converging */
+    TNMC_FLAG_SIGMA_ZERO = 5,    /* informational: a kept singular value was below the numerical rank (exact-chi cases) */
+    TNMC_N_FLAGS = 8
+};
+
+/* Size in bytes of the workspace tnmc_create needs.
+ *   L >= 2, 2 <= chi <= 32, n_dis >= 1, n_samples_max >= 1 (largest n_samples of any later
+ *   tnmc_sample call).  ckpt_stride = 0: keep the full environment stack (all L rows of every
+ *   disorder).  ckpt_stride = k >= 1: keep only every k-th row plus one k-row
+ *   segment and recompute segments inside tnmc_sample (the paper's "streaming protocol",
+ *   PAPER.md:276, done by recomputation instead of disk).  Returns 0 on invalid arguments. */
+size_t tnmc_workspace_bytes(int L, int chi, int n_dis, int n_samples_max, tnmc_prec prec,
+                            int ckpt_stride);
+
+/* Create a context for n_dis disorder realisations.
+ *   Jr, Jd      [dev] int8 (n_dis, L, L), values in {-1, 0, +1}; read (bit-packed into the
+ *               workspace) by a kernel enqueued on the stream; may be freed once the stream has
+ *               passed that point.  Values outside {-1,0,+1} are treated as their sign.
+ *   first_disorder  global index of disorder 0 (enters the Philox counter only)
+ *   workspace   [dev] >= tnmc_workspace_bytes(...) bytes, 256-byte aligned
+ *   cuda_stream a cudaStream_t (NULL = legacy default stream)
+ * Errors: TNMC_EINVAL (L < 2, chi < 2 or > 32, non-finite or negative beta, null pointers,
+ * misaligned workspace), TNMC_ENOMEM (workspace_bytes too small), TNMC_ECUDA. */
+tnmc_status tnmc_create(tnmc_ctx** out, int L, int chi, double beta, int n_dis,
+                        const int8_t* Jr, const int8_t* Jd, uint64_t first_disorder,
+                        int n_samples_max, tnmc_prec prec, int ckpt_stride,
+                        void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Build the boundary-MPS environment stack (steps a-1..a-7 of DESIGN.md).
+ *   logZ [dev] double (n_dis) or NULL:  log Z_chi(d) = logscale_0 + log sum_sigma Psihat_0(sigma).
+ * With ckpt_stride > 0 only the checkpoint rows are kept.  Must precede tnmc_sample. */
+tnmc_status tnmc_build_envs(tnmc_ctx* ctx, double* logZ);
+
+/* Draw n_samples configurations for each of disorders [dis_begin, dis_begin + dis_count).
+ *   seed, sample_offset  Philox indexing (see above)
+ *   cfg_bits [dev] uint32 (dis_count, n_samples, L, W)   out
+ *   logq     [dev] double (dis_count, n_samples)         out: log q(s)
+ * Errors: TNMC_ESTATE before tnmc_build_envs; TNMC_EINVAL on a bad range or
+ * n_samples > n_samples_max. */
+tnmc_status tnmc_sample(tnmc_ctx* ctx, int dis_begin, int dis_count, int n_samples,
+                        uint64_t seed, uint64_t sample_offset,
+                        uint32_t* cfg_bits, double* logq);
+
+/* As tnmc_sample, with the test hooks of DESIGN.md:
+ *   forced_cfg_bits [dev] uint32, same shape as cfg_bits, or NULL.  Teacher forcing: use these
+ *                   spins instead of u < p; log q and probs are still those of the model
+ *                   (cfg_bits receives a copy of the forced spins).
+ *   probs           [dev] double (dis_count, n_samples, L, L) or NULL: q(s_i = +1 | s_<i). */
+tnmc_status tnmc_sample_ex(tnmc_ctx* ctx, int dis_begin, int dis_count, int n_samples,
+                           uint64_t seed, uint64_t sample_offset,
+                           const uint32_t* forced_cfg_bits,
+                           uint32_t* cfg_bits, double* logq, double* probs);
+
+/* Exact energies, Eq. 1:  E = -sum_<ij> J_ij s_i s_j, integer arithmetic on the
+ * packed words (XOR + popcount).
+ *   cfg_bits [dev] uint32 (dis_count, n_samples, L, W)   in
+ *   E        [dev] int32  (dis_count, n_samples)         out */
+tnmc_status tnmc_energy(tnmc_ctx* ctx, int dis_begin, int dis_count, int n_samples,
+                        const uint32_t* cfg_bits, int32_t* E);
+
+/* Independence Metropolis scan, Eq. 10 (readings G15/G16): one chain per
+ * disorder, proposals in sample order; accept iff log u < -beta (E' - E) + log q(s) - log q(s').
+ *   E, logq     [dev] (dis_count, n_samples)  proposals
+ *   seed, step_offset  Philox indexing: draw n of this call uses step index step_offset + n
+ *   cur_logq, cur_E, cur_idx [dev] (dis_count)  in/out chain state; cur_idx < 0 means empty:
+ *               the first proposal then initialises the chain (flag 1, not counted)
+ *   accepted    [dev] uint8 (dis_count, n_samples)  out
+ *   n_accepted  [dev] int64 (dis_count)  out: acceptances of this call
+ *   sum_min1    [dev] double (dis_count) or NULL  out: sum over counted proposals of min(1, ratio) */
+tnmc_status tnmc_metropolis(tnmc_ctx* ctx, int dis_begin, int dis_count, int n_samples,
+                            const int32_t* E, const double* logq,
+                            uint64_t seed, uint64_t step_offset,
+                            double* cur_logq, int32_t* cur_E, int64_t* cur_idx,
+                            uint8_t* accepted, int64_t* n_accepted, double* sum_min1);
+
+/* One whole pass for host callers: copies Jr/Jd (host, int8 (n_dis,L,L)) to the device, builds
+ * the environments, samples, computes energies, runs the Metropolis scan on fresh chains and
+ * copies the results back.  All device memory comes from `workspace`
+ * (>= tnmc_run_host_workspace_bytes).  Synchronises the stream before returning.
+ *   out_cfg_bits [host] uint32 (n_dis, n_samples, L, W) or NULL
+ *   out_E [host] int32, out_logq [host] double, out_accepted [host] uint8: (n_dis, n_samples)
+ *   out_logZ [host] double (n_dis), out_n_accepted [host] int64 (n_dis); any may be NULL. */
+size_t tnmc_run_host_workspace_bytes(int L, int chi, int n_dis, int n_samples, tnmc_prec prec,
+                                     int ckpt_stride);
+tnmc_status tnmc_run_host(int L, int chi, double beta, int n_dis, int n_samples,
+                          const int8_t* Jr_host, const int8_t* Jd_host, uint64_t first_disorder,
+                          uint64_t seed, tnmc_prec prec, int ckpt_stride,
+                          void* workspace, size_t workspace_bytes, void* cuda_stream,
+                          uint32_t* out_cfg_bits, int32_t* out_E, double* out_logq,
+                          uint8_t* out_accepted, double* out_logZ, int64_t* out_n_accepted);
+
+/* Device fault counters -> host_flags_out[TNMC_N_FLAGS] [host].  Synchronises the stream. */
+tnmc_status tnmc_get_flags(tnmc_ctx* ctx, uint64_t* host_flags_out);
+
+/* Test/inspection hook: copy one stored environment row of one disorder to the host in the
+ * paper's layout: out [host] double (L, chi, 2, chi), zero-padded where the bond
+ * is smaller than chi; *logscale_out [host] receives logscale_r (Psi_r = e^logscale Psihat_r).
+ * TNMC_ESTATE if that row is not currently stored (checkpoint mode).  Synchronises. */
+tnmc_status tnmc_get_env_row(tnmc_ctx* ctx, int disorder, int row, double* out,
+                             double* logscale_out);
+
+/* Number of kernels this context has launched so far (bench.py's gpu_launches). */
+uint64_t tnmc_launch_count(const tnmc_ctx* ctx);
+
+const char* tnmc_last_error(const tnmc_ctx* ctx); /* never NULL; ctx may be NULL */
+void tnmc_destroy(tnmc_ctx* ctx);                 /* frees host metadata only */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TNMC_H_ */

@@ -1,0 +1,373 @@
+// tnmc.cu -- C ABI of include/tnmc.h: argument checks, workspace carve-up, kernel launches.
+// Every step of the hot path runs in the kernels of tnmc_build.cuh / tnmc_sample.cuh /
+// tnmc_energy.cuh; nothing here computes on the host and there is no CPU fallback.
+#include <cmath>
+
+#include "tnmc_ctx.cuh"
+
+using namespace tnmc;
+
+static thread_local std::string g_err;   // errors raised without a context
+
+static tnmc_status fail(tnmc_ctx* ctx, tnmc_status st, const std::string& msg) {
+    if (ctx) ctx->err = msg; else g_err = msg;
+    return st;
+}
+static tnmc_status cuda_fail(tnmc_ctx* ctx, cudaError_t e, const char* what) {
+    return fail(ctx, TNMC_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+#define CK(ctx, call)                                                   \
+    do {                                                                \
+        cudaError_t e__ = (call);                                       \
+        if (e__ != cudaSuccess) return cuda_fail(ctx, e__, #call);      \
+    } while (0)
+#define CK_LAUNCH(ctx, name)                                            \
+    do {                                                                \
+        cudaError_t e__ = cudaPeekAtLastError();                        \
+        if (e__ != cudaSuccess) return cuda_fail(ctx, e__, name);       \
+        (ctx)->launches++;                                              \
+    } while (0)
+
+extern "C" size_t tnmc_workspace_bytes(int L, int chi, int n_dis, int n_samples_max, tnmc_prec prec,
+                                       int ckpt_stride) {
+    Plan p;
+    if (prec != TNMC_F64) return 0;
+    if (!make_plan(p, L, chi, n_dis, n_samples_max, ckpt_stride)) return 0;
+    return p.total;
+}
+
+extern "C" tnmc_status tnmc_create(tnmc_ctx** out, int L, int chi, double beta, int n_dis,
+                                   const int8_t* Jr, const int8_t* Jd, uint64_t first_disorder,
+                                   int n_samples_max, tnmc_prec prec, int ckpt_stride,
+                                   void* workspace, size_t workspace_bytes, void* cuda_stream) {
+    if (!out) return fail(nullptr, TNMC_EINVAL, "tnmc_create: out is NULL");
+    *out = nullptr;
+    if (prec != TNMC_F64) return fail(nullptr, TNMC_EINVAL, "tnmc_create: only TNMC_F64 is implemented");
+    if (!Jr || !Jd || !workspace) return fail(nullptr, TNMC_EINVAL, "tnmc_create: NULL pointer");
+    if (!(beta >= 0.0) || !std::isfinite(beta)) return fail(nullptr, TNMC_EINVAL, "tnmc_create: beta must be finite and >= 0");
+    if ((reinterpret_cast<uintptr_t>(workspace) & 255u) != 0) return fail(nullptr, TNMC_EINVAL, "tnmc_create: workspace must be 256-byte aligned");
+    Plan p;
+    if (!make_plan(p, L, chi, n_dis, n_samples_max, ckpt_stride))
+        return fail(nullptr, TNMC_EINVAL, "tnmc_create: need 2 <= L <= 4096, 2 <= chi <= 32, n_dis >= 1, n_samples_max >= 1, ckpt_stride >= 0");
+    if (workspace_bytes < p.total) return fail(nullptr, TNMC_ENOMEM, "tnmc_create: workspace too small");
+    int dev_count = 0;
+    if (cudaGetDeviceCount(&dev_count) != cudaSuccess || dev_count == 0)
+        return fail(nullptr, TNMC_ECUDA, "tnmc_create: no CUDA device (there is no CPU fallback)");
+
+    tnmc_ctx* ctx = new tnmc_ctx();
+    ctx->plan = p;
+    ctx->beta = beta;
+    ctx->first_disorder = first_disorder;
+    ctx->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+    ctx->ws = reinterpret_cast<char*>(workspace);
+
+    auto bail = [&](tnmc_status st) { g_err = ctx->err; delete ctx; return st; };
+    // slot maps -> device
+    std::vector<int> maps((size_t)p.n_maps * L);
+    for (int m = 0; m < p.n_maps; ++m) {
+        const std::vector<int> s = p.slot_map(m);
+        std::memcpy(maps.data() + (size_t)m * L, s.data(), sizeof(int) * L);
+    }
+    cudaError_t e = cudaMemcpyAsync(ctx->at<int>(p.off_maps), maps.data(), sizeof(int) * maps.size(),
+                                    cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);   // `maps` is a host temporary
+    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->at<char>(p.off_flags), 0, sizeof(unsigned long long) * N_FLAGS, ctx->stream);
+    if (e != cudaSuccess) return bail(cuda_fail(ctx, e, "tnmc_create: upload"));
+    {
+        const size_t n_words = (size_t)n_dis * L * p.W;
+        const int threads = 256;
+        const unsigned blocks = (unsigned)((n_words + threads - 1) / threads);
+        pack_couplings_kernel<<<blocks, threads, 0, ctx->stream>>>(Jr, Jd, n_dis, L, p.W, ctx->at<uint32_t>(p.off_masks));
+        e = cudaPeekAtLastError();
+        if (e != cudaSuccess) return bail(cuda_fail(ctx, e, "pack_couplings_kernel"));
+        ctx->launches++;
+    }
+    *out = ctx;
+    return TNMC_OK;
+}
+
+extern "C" const char* tnmc_last_error(const tnmc_ctx* ctx) { return ctx ? ctx->err.c_str() : g_err.c_str(); }
+extern "C" uint64_t tnmc_launch_count(const tnmc_ctx* ctx) { return ctx ? ctx->launches : 0; }
+extern "C" void tnmc_destroy(tnmc_ctx* ctx) { delete ctx; }
+
+// ---------------------------------------------------------------------------------------------
+// launch helpers
+// ---------------------------------------------------------------------------------------------
+template <int P>
+static cudaError_t launch_build_t(const tnmc_ctx* ctx, const BuildArgs& a, int dis_count) {
+    const size_t smem = BuildCfg<P>::smem_bytes(a.L);
+    cudaError_t e = cudaFuncSetAttribute(build_rows_kernel<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    build_rows_kernel<P><<<dis_count, BUILD_THREADS, smem, ctx->stream>>>(a);
+    return cudaPeekAtLastError();
+}
+
+// rows row_hi-1 .. row_lo of disorders [dis_begin, dis_begin+dis_count) using slot map `m`
+static tnmc_status launch_build(tnmc_ctx* ctx, int m, int row_hi, int row_lo, int dis_begin, int dis_count) {
+    if (row_hi <= row_lo) return TNMC_OK;
+    const Plan& p = ctx->plan;
+    BuildArgs a;
+    a.J = ctx->jview();
+    a.beta = ctx->beta; a.L = p.L; a.chi = p.chi; a.dis_begin = dis_begin;
+    a.row_hi = row_hi; a.row_lo = row_lo;
+    a.slot_of_row = ctx->map(m);
+    a.env = ctx->at<double>(p.off_env); a.env_dis_stride = p.env_dis_stride;
+    a.qbuf = ctx->at<double>(p.off_qbuf);
+    a.logscale = ctx->at<double>(p.off_logscale);
+    a.flags = ctx->at<unsigned long long>(p.off_flags);
+    cudaError_t e;
+    if (p.P == 8) e = launch_build_t<8>(ctx, a, dis_count);
+    else if (p.P == 16) e = launch_build_t<16>(ctx, a, dis_count);
+    else e = launch_build_t<32>(ctx, a, dis_count);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "build_rows_kernel");
+    ctx->launches++;
+    return TNMC_OK;
+}
+
+template <int P>
+static cudaError_t launch_sample_t(const tnmc_ctx* ctx, const SampleArgs& a, int tiles, int dis_count) {
+    const int W = (a.L + 31) / 32;
+    const size_t smem = sizeof(double) * SAMPLE_STAGES * 2 * P * P + sizeof(uint32_t) * SAMPLE_CHAINS * W;
+    cudaError_t e = cudaFuncSetAttribute(sample_rows_kernel<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    sample_rows_kernel<P><<<dim3(tiles, dis_count), SAMPLE_THREADS, smem, ctx->stream>>>(a);
+    return cudaPeekAtLastError();
+}
+
+// ---------------------------------------------------------------------------------------------
+// tnmc_build_envs
+// ---------------------------------------------------------------------------------------------
+extern "C" tnmc_status tnmc_build_envs(tnmc_ctx* ctx, double* logZ) {
+    if (!ctx) return fail(nullptr, TNMC_EINVAL, "tnmc_build_envs: ctx is NULL");
+    const Plan& p = ctx->plan;
+    const int* map0 = ctx->map(0);
+    (void)map0;
+    bottom_row_kernel<<<dim3(p.L, p.n_dis), 64, 0, ctx->stream>>>(
+        ctx->jview(), ctx->beta, p.L, p.P, ctx->at<double>(p.off_env), p.env_dis_stride,
+        p.perm_slot(p.L - 1), ctx->at<double>(p.off_logscale));
+    CK_LAUNCH(ctx, "bottom_row_kernel");
+    tnmc_status st = launch_build(ctx, 0, p.L - 1, 0, 0, p.n_dis);
+    if (st != TNMC_OK) return st;
+    double* lz = logZ ? logZ : ctx->at<double>(p.off_logz);
+    const int warps = 4;
+    logz_kernel<<<(p.n_dis + warps - 1) / warps, warps * 32, 0, ctx->stream>>>(
+        p.L, p.chi, p.P, p.n_dis, ctx->at<double>(p.off_env), p.env_dis_stride, p.perm_slot(0),
+        ctx->at<double>(p.off_logscale), lz, ctx->at<unsigned long long>(p.off_flags));
+    CK_LAUNCH(ctx, "logz_kernel");
+    ctx->built = true;
+    return TNMC_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// tnmc_sample / tnmc_sample_ex
+// ---------------------------------------------------------------------------------------------
+static tnmc_status check_range(tnmc_ctx* ctx, const char* who, int dis_begin, int dis_count, int n_samples) {
+    if (!ctx) return fail(nullptr, TNMC_EINVAL, std::string(who) + ": ctx is NULL");
+    if (dis_begin < 0 || dis_count < 1 || dis_begin + dis_count > ctx->plan.n_dis)
+        return fail(ctx, TNMC_EINVAL, std::string(who) + ": disorder range out of bounds");
+    if (n_samples < 1) return fail(ctx, TNMC_EINVAL, std::string(who) + ": n_samples < 1");
+    return TNMC_OK;
+}
+
+extern "C" tnmc_status tnmc_sample_ex(tnmc_ctx* ctx, int dis_begin, int dis_count, int n_samples,
+                                      uint64_t seed, uint64_t sample_offset,
+                                      const uint32_t* forced_cfg_bits,
+                                      uint32_t* cfg_bits, double* logq, double* probs) {
+    tnmc_status st = check_range(ctx, "tnmc_sample", dis_begin, dis_count, n_samples);
+    if (st != TNMC_OK) return st;
+    if (!ctx->built) return fail(ctx, TNMC_ESTATE, "tnmc_sample: call tnmc_build_envs first");
+    const Plan& p = ctx->plan;
+    if (n_samples > p.n_samples_max) return fail(ctx, TNMC_EINVAL, "tnmc_sample: n_samples > n_samples_max");
+    if (!cfg_bits || !logq) return fail(ctx, TNMC_EINVAL, "tnmc_sample: NULL output pointer");
+    SampleArgs a;
+    a.J = ctx->jview();
+    a.beta = ctx->beta; a.L = p.L; a.chi = p.chi;
+    a.dis_begin = dis_begin; a.n_samples = n_samples;
+    a.env = ctx->at<double>(p.off_env); a.env_dis_stride = p.env_dis_stride;
+    a.renv = ctx->at<double>(p.off_renv);
+    a.cfg_bits = cfg_bits; a.forced = forced_cfg_bits; a.logq = logq; a.probs = probs;
+    a.seed_lo = (uint32_t)(seed & 0xffffffffu); a.seed_hi = (uint32_t)(seed >> 32);
+    a.sample_offset = sample_offset; a.first_disorder = ctx->first_disorder;
+    a.flags = ctx->at<unsigned long long>(p.off_flags);
+    const int tiles = (n_samples + SAMPLE_CHAINS - 1) / SAMPLE_CHAINS;
+    for (int j = 0; j < p.n_seg; ++j) {
+        int m = 0;
+        if (p.ckpt > 0) {
+            // recompute the rows of segment j from the first stored row below it (a-6)
+            m = 1 + j;
+            st = launch_build(ctx, m, p.seg_start_row(j), j * p.ckpt + 1, dis_begin, dis_count);
+            if (st != TNMC_OK) return st;
+            a.row_lo = j * p.ckpt; a.row_hi = p.seg_end(j);
+        } else { a.row_lo = 0; a.row_hi = p.L; }
+        a.slot_of_row = ctx->map(m);
+        cudaError_t e;
+        if (p.P == 8) e = launch_sample_t<8>(ctx, a, tiles, dis_count);
+        else if (p.P == 16) e = launch_sample_t<16>(ctx, a, tiles, dis_count);
+        else e = launch_sample_t<32>(ctx, a, tiles, dis_count);
+        if (e != cudaSuccess) return cuda_fail(ctx, e, "sample_rows_kernel");
+        ctx->launches++;
+    }
+    return TNMC_OK;
+}
+
+extern "C" tnmc_status tnmc_sample(tnmc_ctx* ctx, int dis_begin, int dis_count, int n_samples,
+                                   uint64_t seed, uint64_t sample_offset,
+                                   uint32_t* cfg_bits, double* logq) {
+    return tnmc_sample_ex(ctx, dis_begin, dis_count, n_samples, seed, sample_offset, nullptr, cfg_bits, logq, nullptr);
+}
+
+// ---------------------------------------------------------------------------------------------
+// tnmc_energy / tnmc_metropolis
+// ---------------------------------------------------------------------------------------------
+extern "C" tnmc_status tnmc_energy(tnmc_ctx* ctx, int dis_begin, int dis_count, int n_samples,
+                                   const uint32_t* cfg_bits, int32_t* E) {
+    tnmc_status st = check_range(ctx, "tnmc_energy", dis_begin, dis_count, n_samples);
+    if (st != TNMC_OK) return st;
+    if (!cfg_bits || !E) return fail(ctx, TNMC_EINVAL, "tnmc_energy: NULL pointer");
+    const Plan& p = ctx->plan;
+    const long long n_cfg = (long long)dis_count * n_samples;
+    const int warps = 8;
+    const unsigned blocks = (unsigned)((n_cfg + warps - 1) / warps);
+    energy_kernel<<<blocks, warps * 32, 0, ctx->stream>>>(ctx->jview(), p.L, p.W, dis_begin, dis_count,
+                                                          n_samples, cfg_bits, E);
+    CK_LAUNCH(ctx, "energy_kernel");
+    return TNMC_OK;
+}
+
+extern "C" tnmc_status tnmc_metropolis(tnmc_ctx* ctx, int dis_begin, int dis_count, int n_samples,
+                                       const int32_t* E, const double* logq,
+                                       uint64_t seed, uint64_t step_offset,
+                                       double* cur_logq, int32_t* cur_E, int64_t* cur_idx,
+                                       uint8_t* accepted, int64_t* n_accepted, double* sum_min1) {
+    tnmc_status st = check_range(ctx, "tnmc_metropolis", dis_begin, dis_count, n_samples);
+    if (st != TNMC_OK) return st;
+    if (!E || !logq || !cur_logq || !cur_E || !cur_idx || !accepted || !n_accepted)
+        return fail(ctx, TNMC_EINVAL, "tnmc_metropolis: NULL pointer");
+    const int threads = 64;
+    metropolis_kernel<<<(dis_count + threads - 1) / threads, threads, 0, ctx->stream>>>(
+        ctx->beta, dis_begin, dis_count, n_samples, E, logq, (uint32_t)(seed & 0xffffffffu),
+        (uint32_t)(seed >> 32), step_offset, ctx->first_disorder, cur_logq, cur_E,
+        cur_idx, accepted, n_accepted, sum_min1);
+    CK_LAUNCH(ctx, "metropolis_kernel");
+    return TNMC_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// inspection
+// ---------------------------------------------------------------------------------------------
+extern "C" tnmc_status tnmc_get_flags(tnmc_ctx* ctx, uint64_t* host_flags_out) {
+    if (!ctx || !host_flags_out) return fail(ctx, TNMC_EINVAL, "tnmc_get_flags: NULL pointer");
+    CK(ctx, cudaMemcpyAsync(host_flags_out, ctx->at<char>(ctx->plan.off_flags), sizeof(uint64_t) * N_FLAGS,
+                            cudaMemcpyDeviceToHost, ctx->stream));
+    CK(ctx, cudaStreamSynchronize(ctx->stream));
+    return TNMC_OK;
+}
+
+extern "C" tnmc_status tnmc_get_env_row(tnmc_ctx* ctx, int disorder, int row, double* out, double* logscale_out) {
+    if (!ctx || !out) return fail(ctx, TNMC_EINVAL, "tnmc_get_env_row: NULL pointer");
+    const Plan& p = ctx->plan;
+    if (disorder < 0 || disorder >= p.n_dis || row < 0 || row >= p.L)
+        return fail(ctx, TNMC_EINVAL, "tnmc_get_env_row: index out of range");
+    if (!ctx->built) return fail(ctx, TNMC_ESTATE, "tnmc_get_env_row: call tnmc_build_envs first");
+    const int slot = p.perm_slot(row);
+    if (slot < 0) return fail(ctx, TNMC_ESTATE, "tnmc_get_env_row: row is not kept in checkpoint mode");
+    // stage through the (currently idle) Q scratch of this disorder
+    double* tmp = ctx->at<double>(p.off_qbuf) + (size_t)disorder * p.L * p.qsz;
+    const double* src = ctx->at<double>(p.off_env) + (size_t)disorder * p.env_dis_stride + (size_t)slot * p.L * p.tsz;
+    export_row_kernel<<<p.L, 128, 0, ctx->stream>>>(p.L, p.chi, p.P, src, tmp);
+    CK_LAUNCH(ctx, "export_row_kernel");
+    CK(ctx, cudaMemcpyAsync(out, tmp, sizeof(double) * (size_t)p.L * p.chi * 2 * p.chi, cudaMemcpyDeviceToHost, ctx->stream));
+    if (logscale_out)
+        CK(ctx, cudaMemcpyAsync(logscale_out, ctx->at<double>(p.off_logscale) + (size_t)disorder * p.L + row,
+                                sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    CK(ctx, cudaStreamSynchronize(ctx->stream));
+    return TNMC_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// tnmc_run_host: the whole pass for callers with host buffers
+// ---------------------------------------------------------------------------------------------
+namespace {
+struct HostPlan {
+    size_t off_jr, off_jd, off_cfg, off_E, off_logq, off_acc, off_logz, off_cq, off_ce, off_ci, off_nacc,
+           off_ctx, ctx_bytes, total;
+};
+bool make_host_plan(HostPlan& h, int L, int chi, int n_dis, int n_samples, int ckpt) {
+    Plan p;
+    if (!make_plan(p, L, chi, n_dis, n_samples, ckpt)) return false;
+    const size_t nc = (size_t)n_dis * n_samples;
+    size_t o = 0;
+    h.off_jr = o;   o = align_up(o + (size_t)n_dis * L * L);
+    h.off_jd = o;   o = align_up(o + (size_t)n_dis * L * L);
+    h.off_cfg = o;  o = align_up(o + sizeof(uint32_t) * nc * L * p.W);
+    h.off_E = o;    o = align_up(o + sizeof(int32_t) * nc);
+    h.off_logq = o; o = align_up(o + sizeof(double) * nc);
+    h.off_acc = o;  o = align_up(o + nc);
+    h.off_logz = o; o = align_up(o + sizeof(double) * n_dis);
+    h.off_cq = o;   o = align_up(o + sizeof(double) * n_dis);
+    h.off_ce = o;   o = align_up(o + sizeof(int32_t) * n_dis);
+    h.off_ci = o;   o = align_up(o + sizeof(int64_t) * n_dis);
+    h.off_nacc = o; o = align_up(o + sizeof(int64_t) * n_dis);
+    h.off_ctx = o;  h.ctx_bytes = p.total; o = align_up(o + p.total);
+    h.total = o;
+    return true;
+}
+}  // namespace
+
+extern "C" size_t tnmc_run_host_workspace_bytes(int L, int chi, int n_dis, int n_samples, tnmc_prec prec,
+                                                int ckpt_stride) {
+    HostPlan h;
+    if (prec != TNMC_F64 || !make_host_plan(h, L, chi, n_dis, n_samples, ckpt_stride)) return 0;
+    return h.total;
+}
+
+extern "C" tnmc_status tnmc_run_host(int L, int chi, double beta, int n_dis, int n_samples,
+                                     const int8_t* Jr_host, const int8_t* Jd_host, uint64_t first_disorder,
+                                     uint64_t seed, tnmc_prec prec, int ckpt_stride,
+                                     void* workspace, size_t workspace_bytes, void* cuda_stream,
+                                     uint32_t* out_cfg_bits, int32_t* out_E, double* out_logq,
+                                     uint8_t* out_accepted, double* out_logZ, int64_t* out_n_accepted) {
+    HostPlan h;
+    if (prec != TNMC_F64 || !make_host_plan(h, L, chi, n_dis, n_samples, ckpt_stride))
+        return fail(nullptr, TNMC_EINVAL, "tnmc_run_host: bad sizes");
+    if (!Jr_host || !Jd_host || !workspace) return fail(nullptr, TNMC_EINVAL, "tnmc_run_host: NULL pointer");
+    if (workspace_bytes < h.total) return fail(nullptr, TNMC_ENOMEM, "tnmc_run_host: workspace too small");
+    char* ws = reinterpret_cast<char*>(workspace);
+    cudaStream_t s = reinterpret_cast<cudaStream_t>(cuda_stream);
+    const size_t nj = (size_t)n_dis * L * L, nc = (size_t)n_dis * n_samples;
+    const int W = (L + 31) / 32;
+    CK(nullptr, cudaMemcpyAsync(ws + h.off_jr, Jr_host, nj, cudaMemcpyHostToDevice, s));
+    CK(nullptr, cudaMemcpyAsync(ws + h.off_jd, Jd_host, nj, cudaMemcpyHostToDevice, s));
+    tnmc_ctx* ctx = nullptr;
+    tnmc_status st = tnmc_create(&ctx, L, chi, beta, n_dis, reinterpret_cast<int8_t*>(ws + h.off_jr),
+                                 reinterpret_cast<int8_t*>(ws + h.off_jd), first_disorder, n_samples, prec,
+                                 ckpt_stride, ws + h.off_ctx, h.ctx_bytes, cuda_stream);
+    if (st != TNMC_OK) return st;
+    auto done = [&](tnmc_status r) { if (r != TNMC_OK) g_err = ctx->err; tnmc_destroy(ctx); return r; };
+    uint32_t* cfg = reinterpret_cast<uint32_t*>(ws + h.off_cfg);
+    int32_t* E = reinterpret_cast<int32_t*>(ws + h.off_E);
+    double* lq = reinterpret_cast<double*>(ws + h.off_logq);
+    uint8_t* acc = reinterpret_cast<uint8_t*>(ws + h.off_acc);
+    double* lz = reinterpret_cast<double*>(ws + h.off_logz);
+    double* cq = reinterpret_cast<double*>(ws + h.off_cq);
+    int32_t* ce = reinterpret_cast<int32_t*>(ws + h.off_ce);
+    int64_t* ci = reinterpret_cast<int64_t*>(ws + h.off_ci);
+    int64_t* na = reinterpret_cast<int64_t*>(ws + h.off_nacc);
+    if ((st = tnmc_build_envs(ctx, lz)) != TNMC_OK) return done(st);
+    if ((st = tnmc_sample(ctx, 0, n_dis, n_samples, seed, 0, cfg, lq)) != TNMC_OK) return done(st);
+    if ((st = tnmc_energy(ctx, 0, n_dis, n_samples, cfg, E)) != TNMC_OK) return done(st);
+    cudaError_t e = cudaMemsetAsync(ci, 0xff, sizeof(int64_t) * n_dis, s);   // cur_idx = -1: empty chains
+    if (e == cudaSuccess) e = cudaMemsetAsync(cq, 0, sizeof(double) * n_dis, s);
+    if (e == cudaSuccess) e = cudaMemsetAsync(ce, 0, sizeof(int32_t) * n_dis, s);
+    if (e != cudaSuccess) return done(cuda_fail(ctx, e, "tnmc_run_host: memset"));
+    if ((st = tnmc_metropolis(ctx, 0, n_dis, n_samples, E, lq, seed, 0, cq, ce, ci, acc, na, nullptr)) != TNMC_OK) return done(st);
+    if (out_cfg_bits && e == cudaSuccess) e = cudaMemcpyAsync(out_cfg_bits, cfg, sizeof(uint32_t) * nc * L * W, cudaMemcpyDeviceToHost, s);
+    if (out_E && e == cudaSuccess) e = cudaMemcpyAsync(out_E, E, sizeof(int32_t) * nc, cudaMemcpyDeviceToHost, s);
+    if (out_logq && e == cudaSuccess) e = cudaMemcpyAsync(out_logq, lq, sizeof(double) * nc, cudaMemcpyDeviceToHost, s);
+    if (out_accepted && e == cudaSuccess) e = cudaMemcpyAsync(out_accepted, acc, nc, cudaMemcpyDeviceToHost, s);
+    if (out_logZ && e == cudaSuccess) e = cudaMemcpyAsync(out_logZ, lz, sizeof(double) * n_dis, cudaMemcpyDeviceToHost, s);
+    if (out_n_accepted && e == cudaSuccess) e = cudaMemcpyAsync(out_n_accepted, na, sizeof(int64_t) * n_dis, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) return done(cuda_fail(ctx, e, "tnmc_run_host: copy back"));
+    return done(TNMC_OK);
+}

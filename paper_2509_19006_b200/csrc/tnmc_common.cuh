@@ -1,0 +1,113 @@
+// tnmc_common.cuh -- layouts, Philox4x32-10, fault counters shared by the CUDA kernels.
+// (Part of the product path; shares nothing with oracle/.)
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace tnmc {
+
+// ---------------------------------------------------------------------------------------------
+// Fault counters (include/tnmc.h TNMC_FLAG_*)
+// ---------------------------------------------------------------------------------------------
+enum { FLAG_RHO_ZERO = 0, FLAG_NONFINITE = 1, FLAG_LOGZ_NONPOS = 2, FLAG_NEAR_THRESHOLD = 3,
+       FLAG_JACOBI_LIMIT = 4, FLAG_SIGMA_ZERO = 5, N_FLAGS = 8 };
+
+__device__ __forceinline__ void raise_flag(unsigned long long* flags, int which) {
+    atomicAdd(flags + which, 1ull);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Environment site-tensor layout in HBM ("fragment order").
+//
+// A stored site tensor is A[i][a][j] (left bond i, spin a, right bond j), zero
+// padded to P x 2 x P with P = 8, 16 or 32 (the smallest of these >= chi).  It is stored so that
+// the left sampling sweep (contraction over i) can feed it to
+// mma.sync.m8n8k4.f64 as the B operand with one conflict-free 8-byte shared-memory load per lane:
+//   k-tile kt holds the four left-bond indices i = 8*(kt/2) + 2*q + (kt%2), q = 0..3
+//   n-tile nt holds the eight columns (a, j) with a = nt / (P/8), j = 8*(nt % (P/8)) + g, g = 0..7
+//   element offset = ((kt * NT + nt) * 32 + g*4 + q),  NT = P/4,  lane = g*4 + q.
+// The odd/even split of i over two k-tiles is what lets the accumulator fragment of one site
+// (lane q holds columns 2q, 2q+1 of each n-tile) be used, unshuffled, as the A fragment of the
+// next site.
+// ---------------------------------------------------------------------------------------------
+__host__ __device__ __forceinline__ int pad_chi(int chi) { return chi <= 8 ? 8 : (chi <= 16 ? 16 : 32); }
+
+__host__ __device__ __forceinline__ int env_off(int P, int i, int a, int j) {
+    const int kt = 2 * (i >> 3) + (i & 1);
+    const int q = (i & 7) >> 1;
+    const int nt = a * (P >> 3) + (j >> 3);
+    const int g = j & 7;
+    return ((kt * (P >> 2) + nt) * 32 + g * 4 + q);
+}
+
+// Bond dimension left of column c (c = 0..L) of the stored row r after compression (P-C2):
+// min(chi, 2^min(c, L-c), 2^(L-r)); 1 at the two ends.  Closed form of the recurrences
+//   q_{c+1} = min(2 q_c, D'_{c+1}),  k_c = min(chi, q_c, 2 k_{c+1})
+// (checked against them by tests/test_host_logic.py).
+__host__ __device__ __forceinline__ int row_bond(int L, int chi, int r, int c) {
+    if (c <= 0 || c >= L) return 1;
+    int e = c < L - c ? c : L - c;
+    if (L - r < e) e = L - r;
+    if (e >= 6) return chi;   // chi <= 32 < 2^6
+    const int v = 1 << e;
+    return v < chi ? v : chi;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11), restated from the published algorithm.
+// Reading R of DESIGN.md: key = (seed lo, seed hi), counter = (site, sample, disorder, tag).
+// ---------------------------------------------------------------------------------------------
+__host__ __device__ __forceinline__ void philox_round(uint32_t& c0, uint32_t& c1, uint32_t& c2,
+                                                      uint32_t& c3, uint32_t k0, uint32_t k1) {
+    const uint64_t p0 = (uint64_t)0xD2511F53u * c0;
+    const uint64_t p1 = (uint64_t)0xCD9E8D57u * c2;
+    const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
+    const uint32_t n1 = (uint32_t)p1;
+    const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+    const uint32_t n3 = (uint32_t)p0;
+    c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+}
+
+// 53-bit uniform in [0,1) from the first two output words.
+__host__ __device__ __forceinline__ double philox_uniform(uint32_t c0, uint32_t c1, uint32_t c2,
+                                                          uint32_t c3, uint32_t k0, uint32_t k1) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        philox_round(c0, c1, c2, c3, k0, k1);
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    const uint64_t m = ((uint64_t)c0 << 21) | (uint64_t)(c1 >> 11);
+    return (double)m * 1.1102230246251565e-16;  // 2^-53
+}
+
+enum { TAG_SPIN = 0, TAG_METROPOLIS = 1 };
+
+// ---------------------------------------------------------------------------------------------
+// Bit-packed couplings: for every disorder and row, W = ceil(L/32) words of each mask.
+//   jr_neg bit c: Jr[r][c] < 0     jr_nz bit c: Jr[r][c] != 0
+//   jd_neg bit c: Jd[r][c] < 0     jd_nz bit c: Jd[r][c] != 0
+// stored as masks[(which * n_dis + d) * L * W + r * W + w], which = 0..3 in that order.
+// ---------------------------------------------------------------------------------------------
+enum { M_JR_NEG = 0, M_JR_NZ = 1, M_JD_NEG = 2, M_JD_NZ = 3 };
+
+struct JView {
+    const uint32_t* masks;
+    int n_dis, L, W;
+    __device__ __forceinline__ const uint32_t* row(int which, int d, int r) const {
+        return masks + ((size_t)which * n_dis + d) * (size_t)L * W + (size_t)r * W;
+    }
+    // coupling value in {-1,0,+1}
+    __device__ __forceinline__ int jr(int d, int r, int c) const {
+        const uint32_t nz = row(M_JR_NZ, d, r)[c >> 5] >> (c & 31) & 1u;
+        const uint32_t ng = row(M_JR_NEG, d, r)[c >> 5] >> (c & 31) & 1u;
+        return nz ? (ng ? -1 : 1) : 0;
+    }
+    __device__ __forceinline__ int jd(int d, int r, int c) const {
+        const uint32_t nz = row(M_JD_NZ, d, r)[c >> 5] >> (c & 31) & 1u;
+        const uint32_t ng = row(M_JD_NEG, d, r)[c >> 5] >> (c & 31) & 1u;
+        return nz ? (ng ? -1 : 1) : 0;
+    }
+};
+
+}  // namespace tnmc

@@ -1,0 +1,111 @@
+// tnmc_ctx.cuh -- host-side context: workspace carve-up and the environment-stack policy (a-6).
+#pragma once
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/tnmc.h"
+#include "tnmc_build.cuh"
+#include "tnmc_common.cuh"
+#include "tnmc_energy.cuh"
+#include "tnmc_sample.cuh"
+
+namespace tnmc {
+
+inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+// Environment-stack policy.
+//   ckpt == 0: every row r lives in slot r.
+//   ckpt == k: permanent slots hold rows 0, k, 2k, ... ("checkpoints") and the bottom row L-1;
+//              max(k-1, 2) further slots hold the rows of the segment being sampled (and serve as
+//              the ping-pong pair of the first pass).  Segment j = rows [jk, min((j+1)k, L)).
+struct Plan {
+    int L = 0, chi = 0, P = 0, W = 0, n_dis = 0, n_samples_max = 0, ckpt = 0;
+    int n_seg = 1, n_slots = 0, n_seg_slots = 0, n_maps = 1, tiles = 1;
+    size_t tsz = 0;                 // doubles per site tensor
+    size_t env_dis_stride = 0;      // doubles per disorder
+    size_t qsz = 0;                 // doubles per site of the Q scratch
+    // byte offsets into the workspace
+    size_t off_masks = 0, off_maps = 0, off_flags = 0, off_logscale = 0, off_logz = 0, off_env = 0,
+           off_qbuf = 0, off_renv = 0, total = 0;
+
+    int ckpt_slot(int j) const { return j; }
+    int bottom_slot() const { return n_seg; }
+    int seg_slot(int i) const { return n_seg + 1 + i; }
+    // permanent slot of row r, or -1
+    int perm_slot(int r) const {
+        if (ckpt == 0) return r;
+        if (r == L - 1) return bottom_slot();
+        if (r % ckpt == 0) return ckpt_slot(r / ckpt);
+        return -1;
+    }
+    // slot map m: m == 0 first pass; m == 1 + j: segment j (checkpoint mode only)
+    std::vector<int> slot_map(int m) const {
+        std::vector<int> s(L, -1);
+        for (int r = 0; r < L; ++r) {
+            const int p = perm_slot(r);
+            if (p >= 0) { s[r] = p; continue; }
+            if (m == 0) s[r] = seg_slot(r & 1);
+            else {
+                const int j = m - 1;
+                if (r > j * ckpt && r < (j + 1) * ckpt) s[r] = seg_slot(r - j * ckpt - 1);
+            }
+        }
+        return s;
+    }
+    // first stored row at or below the end of segment j: where its recomputation starts
+    int seg_start_row(int j) const { const int h = (j + 1) * ckpt; return h <= L - 1 ? h : L - 1; }
+    int seg_end(int j) const { const int h = (j + 1) * ckpt; return h < L ? h : L; }
+};
+
+inline bool make_plan(Plan& p, int L, int chi, int n_dis, int n_samples_max, int ckpt) {
+    if (L < 2 || L > 4096 || chi < 2 || chi > 32 || n_dis < 1 || n_samples_max < 1 || ckpt < 0) return false;
+    if (ckpt >= L) ckpt = 0;
+    p.L = L; p.chi = chi; p.P = pad_chi(chi); p.W = (L + 31) / 32; p.n_dis = n_dis;
+    p.n_samples_max = n_samples_max; p.ckpt = ckpt;
+    p.tsz = (size_t)2 * p.P * p.P;
+    if (ckpt == 0) { p.n_seg = 1; p.n_seg_slots = 0; p.n_slots = L; p.n_maps = 1; }
+    else {
+        p.n_seg = (L + ckpt - 1) / ckpt;
+        p.n_seg_slots = ckpt - 1 > 2 ? ckpt - 1 : 2;
+        p.n_slots = p.n_seg + 1 + p.n_seg_slots;
+        p.n_maps = 1 + p.n_seg;
+    }
+    p.env_dis_stride = (size_t)p.n_slots * L * p.tsz;
+    p.qsz = (size_t)(4 * p.P + 1) * (2 * p.P);
+    p.tiles = (n_samples_max + SAMPLE_CHAINS - 1) / SAMPLE_CHAINS;
+    size_t o = 0;
+    p.off_masks = o;    o = align_up(o + sizeof(uint32_t) * 4 * (size_t)n_dis * L * p.W);
+    p.off_maps = o;     o = align_up(o + sizeof(int) * (size_t)p.n_maps * L);
+    p.off_flags = o;    o = align_up(o + sizeof(unsigned long long) * N_FLAGS);
+    p.off_logscale = o; o = align_up(o + sizeof(double) * (size_t)n_dis * L);
+    p.off_logz = o;     o = align_up(o + sizeof(double) * (size_t)n_dis);
+    p.off_env = o;      o = align_up(o + sizeof(double) * (size_t)n_dis * p.env_dis_stride);
+    p.off_qbuf = o;     o = align_up(o + sizeof(double) * (size_t)n_dis * L * p.qsz);
+    p.off_renv = o;     o = align_up(o + sizeof(double) * (size_t)n_dis * p.tiles * L * SAMPLE_CHAINS * p.P);
+    p.total = o;
+    return true;
+}
+
+}  // namespace tnmc
+
+struct tnmc_ctx {
+    tnmc::Plan plan;
+    double beta = 0.0;
+    uint64_t first_disorder = 0;
+    cudaStream_t stream = nullptr;
+    char* ws = nullptr;
+    bool built = false;
+    uint64_t launches = 0;
+    std::string err;
+
+    template <class T> T* at(size_t off) const { return reinterpret_cast<T*>(ws + off); }
+    tnmc::JView jview() const {
+        tnmc::JView v;
+        v.masks = at<uint32_t>(plan.off_masks);
+        v.n_dis = plan.n_dis; v.L = plan.L; v.W = plan.W;
+        return v;
+    }
+    const int* map(int m) const { return at<int>(plan.off_maps) + (size_t)m * plan.L; }
+};

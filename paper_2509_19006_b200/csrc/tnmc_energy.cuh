@@ -1,0 +1,88 @@
+// tnmc_energy.cuh -- exact +-J energy (a-10, Eq. 1) and the independence
+// Metropolis scan (a-11, Eq. 10).
+#pragma once
+#include "tnmc_common.cuh"
+
+namespace tnmc {
+
+// E = -sum_<ij> J_ij s_i s_j on bit-packed rows.  For a bond with spins differing (x = 1) or not
+// and coupling negative (n = 1) or not, J s s' = 1 - 2 (x ^ n); so with `nz` the mask of present
+// bonds,  sum J s s' = popc(nz) - 2 popc((x ^ n) & nz).  One warp per configuration; lane l
+// takes words l, l+32, ... of the (L x W)-word configuration, so loads are fully coalesced.
+__global__ void energy_kernel(JView J, int L, int W, int dis_begin, int dis_count, int n_samples,
+                              const uint32_t* __restrict__ cfg, int32_t* __restrict__ E) {
+    const long long wid = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    const long long n_cfg = (long long)dis_count * n_samples;
+    if (wid >= n_cfg) return;
+    const int lane = threadIdx.x & 31;
+    const int dl = (int)(wid / n_samples);
+    const int d = dis_begin + dl;
+    const uint32_t* s = cfg + (size_t)wid * L * W;
+    const uint32_t* rn = J.row(M_JR_NEG, d, 0);
+    const uint32_t* rz = J.row(M_JR_NZ, d, 0);
+    const uint32_t* dn = J.row(M_JD_NEG, d, 0);
+    const uint32_t* dz = J.row(M_JD_NZ, d, 0);
+    int acc = 0;
+    const int n_words = L * W;
+    for (int i = lane; i < n_words; i += 32) {
+        const int w = i % W, r = i / W;
+        const uint32_t cur = s[i];
+        // right bonds: spin c against spin c+1 (bit 0 of the next word carries over)
+        uint32_t nxt = cur >> 1;
+        if (w + 1 < W) nxt |= s[i + 1] << 31;
+        const uint32_t zr = rz[i];
+        acc += __popc(zr) - 2 * __popc(((cur ^ nxt) ^ rn[i]) & zr);
+        // down bonds: row r against row r+1
+        if (r + 1 < L) {
+            const uint32_t zd = dz[i];
+            acc += __popc(zd) - 2 * __popc(((cur ^ s[i + W]) ^ dn[i]) & zd);
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if (lane == 0) E[wid] = -acc;
+}
+
+// One thread per disorder: sequential scan over its proposals (readings G15/G16).
+__global__ void metropolis_kernel(double beta, int dis_begin, int dis_count, int n_samples,
+                                  const int32_t* __restrict__ E, const double* __restrict__ logq,
+                                  uint32_t seed_lo, uint32_t seed_hi, uint64_t step_offset,
+                                  uint64_t first_disorder,
+                                  double* cur_logq, int32_t* cur_E, int64_t* cur_idx,
+                                  uint8_t* accepted, int64_t* n_accepted, double* sum_min1) {
+    const int dl = blockIdx.x * blockDim.x + threadIdx.x;
+    if (dl >= dis_count) return;
+    const uint32_t ctr_dis = (uint32_t)(first_disorder + (uint64_t)(dis_begin + dl));
+    double cq = cur_logq[dl];
+    int ce = cur_E[dl];
+    long long ci = cur_idx[dl];
+    long long nacc = 0;
+    double smin = 0.0;
+    const size_t base = (size_t)dl * n_samples;
+    for (int n = 0; n < n_samples; ++n) {
+        const int en = E[base + n];
+        const double qn = logq[base + n];
+        const uint64_t stepi = step_offset + (uint64_t)n;
+        if (ci < 0) {                 // empty chain: first proposal initialises it (not counted)
+            ce = en; cq = qn; ci = (long long)stepi;
+            accepted[base + n] = 1;
+            continue;
+        }
+        const double logA = -beta * (double)(en - ce) + cq - qn;     // Eq. 10 in log form
+        smin += logA < 0.0 ? exp(logA) : 1.0;
+        const double u = philox_uniform(0u, (uint32_t)stepi, ctr_dis, TAG_METROPOLIS, seed_lo, seed_hi);
+        const double logu = u > 0.0 ? log(u) : -INFINITY;
+        if (logu < logA) {
+            ce = en; cq = qn; ci = (long long)stepi;
+            accepted[base + n] = 1;
+            ++nacc;
+        } else {
+            accepted[base + n] = 0;
+        }
+    }
+    cur_logq[dl] = cq; cur_E[dl] = ce; cur_idx[dl] = ci;
+    n_accepted[dl] = nacc;
+    if (sum_min1 != nullptr) sum_min1[dl] = smin;
+}
+
+}  // namespace tnmc

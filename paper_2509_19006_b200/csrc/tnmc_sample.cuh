@@ -1,0 +1,345 @@
+// tnmc_sample.cuh -- row-by-row ancestral sampling (steps a-8, a-9 of DESIGN.md;
+// SamplerIsing._sample_row).
+//
+// One CTA = one disorder x one tile of chains (samples); it walks all rows of its range with no
+// inter-CTA dependency (chains never interact).  Per row: the right-environment
+// sweep writes R_c to a CTA-private scratch in HBM, the left sweep
+// reads it back.  Both sweeps are (chains x chi) x (chi x 2chi) products, run
+// on the FP64 tensor pipe with mma.sync.m8n8k4.f64: 8 chains form the M dimension of one tile,
+// the site tensor (shared by every chain of the disorder) is the B operand, staged through
+// shared memory with a cp.async ring that runs ahead across sweeps and rows.
+//
+// Fragment bookkeeping (see tnmc_common.cuh): with lane = 4*g + q,
+//   A fragment (8x4):  lane holds  V[chain g][k-slot q]          of k-tile kt
+//   B fragment (4x8):  lane holds  T[k-slot q][column g]         of (kt, nt)
+//   C fragment (8x8):  lane holds  out[chain g][2q], [2q+1]      of n-tile nt
+// and k-tile kt, slot q  <->  bond index 8*(kt/2) + 2q + (kt%2), so the C fragments of one site
+// are, register for register, the A fragments of the next.
+#pragma once
+#include "tnmc_common.cuh"
+
+namespace tnmc {
+
+constexpr int SAMPLE_WARPS = 8;
+constexpr int SAMPLE_THREADS = SAMPLE_WARPS * 32;
+constexpr int SAMPLE_MT = 2;                                   // 8-chain M tiles per warp
+constexpr int SAMPLE_CHAINS = SAMPLE_WARPS * SAMPLE_MT * 8;    // chains per CTA
+constexpr int SAMPLE_STAGES = 3;
+
+struct SampleArgs {
+    JView J;
+    double beta;
+    int L, chi;
+    int dis_begin, n_samples;
+    int row_lo, row_hi;              // rows [row_lo, row_hi)
+    const int* slot_of_row;          // [L] device
+    const double* env;
+    size_t env_dis_stride;
+    double* renv;                    // scratch: per CTA  L * SAMPLE_CHAINS * P doubles
+    uint32_t* cfg_bits;              // (dis_count, n_samples, L, W)
+    const uint32_t* forced;          // or nullptr
+    double* logq;                    // (dis_count, n_samples): accumulated over row ranges
+    double* probs;                   // (dis_count, n_samples, L, L) or nullptr
+    uint32_t seed_lo, seed_hi;
+    uint64_t sample_offset, first_disorder;
+    unsigned long long* flags;
+};
+
+__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" :: "r"(s), "l"(gmem_src));
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int N> __device__ __forceinline__ void cp_async_wait() {
+    asm volatile("cp.async.wait_group %0;\n" :: "n"(N));
+}
+
+__device__ __forceinline__ double quad_sum(double v) {
+    v += __shfl_xor_sync(0xffffffffu, v, 1);
+    v += __shfl_xor_sync(0xffffffffu, v, 2);
+    return v;
+}
+
+template <int P>
+__global__ void __launch_bounds__(SAMPLE_THREADS, 1) sample_rows_kernel(const SampleArgs args) {
+    constexpr int KT = P / 4;        // k tiles
+    constexpr int NT = P / 4;        // n tiles (2P / 8)
+    constexpr int JT = P / 8;        // 8-wide tiles per spin slice
+    constexpr int MT = SAMPLE_MT;
+    constexpr int TSZ = 2 * P * P;
+    extern __shared__ __align__(16) double smem[];
+    double* sT = smem;                                                    // SAMPLE_STAGES * TSZ
+    uint32_t* sBits = reinterpret_cast<uint32_t*>(smem + SAMPLE_STAGES * TSZ);  // [SAMPLE_CHAINS][W] previous row
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int g = lane >> 2, q = lane & 3;
+    const int L = args.L, W = (L + 31) >> 5;
+    const int dl = blockIdx.y;                       // local disorder index (output indexing)
+    const int d = args.dis_begin + dl;               // ctx disorder index (env / J indexing)
+    const int tile = blockIdx.x;
+    const double beta = args.beta;
+    const double eb = exp(beta), emb = exp(-beta);
+    const double* env_d = args.env + (size_t)d * args.env_dis_stride;
+    double* renv = args.renv + ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * (size_t)L * SAMPLE_CHAINS * P;
+
+    // chain handled as M-tile mt, row g of this warp
+    int chain_local[MT];      // index within the CTA
+    long long samp[MT];       // sample index within this call (may be >= n_samples: inactive)
+#pragma unroll
+    for (int mt = 0; mt < MT; ++mt) {
+        chain_local[mt] = (warp * MT + mt) * 8 + g;
+        samp[mt] = (long long)tile * SAMPLE_CHAINS + chain_local[mt];
+    }
+    // the "owner" lane of chain (mt = q, g) does that chain's scalar work
+    const bool owner = q < MT;
+    const int own_local = (warp * MT + (owner ? q : 0)) * 8 + g;
+    const long long own_samp = (long long)tile * SAMPLE_CHAINS + own_local;
+    const bool own_active = owner && own_samp < args.n_samples;
+    const size_t own_out = (size_t)dl * args.n_samples + (size_t)(own_active ? own_samp : 0);
+    const uint32_t ctr_samp = (uint32_t)(args.sample_offset + (uint64_t)own_samp);
+    const uint32_t ctr_dis = (uint32_t)(args.first_disorder + (uint64_t)d);
+
+    double logq = 0.0;
+    if (own_active && args.row_lo > 0) logq = args.logq[own_out];
+
+    // previous-row bits of this CTA's chains -> shared (zero for row 0: reading G9, no upper row)
+    for (int t = tid; t < SAMPLE_CHAINS * W; t += SAMPLE_THREADS) {
+        const int cl = t / W, w = t % W;
+        const long long s = (long long)tile * SAMPLE_CHAINS + cl;
+        uint32_t v = 0;
+        if (args.row_lo > 0 && s < args.n_samples)
+            v = args.cfg_bits[(((size_t)dl * args.n_samples + s) * L + (args.row_lo - 1)) * W + w];
+        sBits[t] = v;
+    }
+
+    // ---- tensor stream: per row the right sweep consumes sites L-1..1, the left sweep sites 0..L-1
+    const int steps_per_row = 2 * L - 1;
+    const int n_rows = args.row_hi - args.row_lo;
+    const long long total_steps = (long long)n_rows * steps_per_row;
+    auto issue_prefetch = [&](long long s) {
+        if (s < total_steps) {
+            const int rr = args.row_lo + (int)(s / steps_per_row);
+            const int t = (int)(s % steps_per_row);
+            const int site = t < L - 1 ? (L - 1 - t) : (t - (L - 1));
+            const double* src = env_d + ((size_t)args.slot_of_row[rr] * L + site) * TSZ;
+            double* dst = sT + (size_t)(s % SAMPLE_STAGES) * TSZ;
+            for (int o = tid * 2; o < TSZ; o += SAMPLE_THREADS * 2) cp_async16(dst + o, src + o);
+        }
+        cp_async_commit();
+    };
+    for (int s = 0; s < SAMPLE_STAGES - 1; ++s) issue_prefetch(s);
+
+    long long step = 0;
+    for (int r = args.row_lo; r < args.row_hi; ++r) {
+        const bool has_up = r > 0;
+        // ============================================================ right sweep
+        double vf[MT][KT];          // current environment as A fragments
+#pragma unroll
+        for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+            for (int kt = 0; kt < KT; ++kt) vf[mt][kt] = (kt == 0 && q == 0) ? 1.0 : 0.0;
+        {   // R_{L-1} = [1]
+#pragma unroll
+            for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+                for (int jt = 0; jt < JT; ++jt) {
+                    double2 v = make_double2((jt == 0 && q == 0) ? 1.0 : 0.0, 0.0);
+                    double2* dst = reinterpret_cast<double2*>(
+                        renv + ((((size_t)(L - 1) * SAMPLE_WARPS + warp) * MT + mt) * JT + jt) * 64) + lane;
+                    *dst = v;
+                }
+        }
+        uint32_t upw[MT] = {0u, 0u};
+        uint32_t jneg = 0, jnz = 0;
+        const uint32_t* jd_neg = has_up ? args.J.row(M_JD_NEG, d, r - 1) : nullptr;
+        const uint32_t* jd_nz = has_up ? args.J.row(M_JD_NZ, d, r - 1) : nullptr;
+        int cur_word = -1;
+        for (int col = L - 2; col >= 0; --col, ++step) {
+            cp_async_wait<SAMPLE_STAGES - 2>();
+            __syncthreads();
+            issue_prefetch(step + SAMPLE_STAGES - 1);
+            const double* T = sT + (size_t)(step % SAMPLE_STAGES) * TSZ;   // tensor of site col+1
+            const int site = col + 1;
+            if ((site >> 5) != cur_word) {
+                cur_word = site >> 5;
+                if (has_up) {
+                    jneg = jd_neg[cur_word]; jnz = jd_nz[cur_word];
+#pragma unroll
+                    for (int mt = 0; mt < MT; ++mt) upw[mt] = sBits[chain_local[mt] * W + cur_word];
+                }
+            }
+            double acc[MT][NT][2];
+#pragma unroll
+            for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+                for (int nt = 0; nt < NT; ++nt) { acc[mt][nt][0] = 0.0; acc[mt][nt][1] = 0.0; }
+            // out[chain][(a,i)] = sum_j T[i][a][j] R[chain][j]
+#pragma unroll
+            for (int kt = 0; kt < KT; ++kt) {
+                const int j = 8 * (kt >> 1) + 2 * q + (kt & 1);
+#pragma unroll
+                for (int nt = 0; nt < NT; ++nt) {
+                    const int a = nt / JT, i = 8 * (nt % JT) + g;
+                    const double b = T[env_off(P, i, a, j)];
+#pragma unroll
+                    for (int mt = 0; mt < MT; ++mt) dmma884(acc[mt][nt][0], acc[mt][nt][1], vf[mt][kt], b);
+                }
+            }
+            // weights of the up bond for the two spin values
+            const int bit = site & 31;
+            const int jsign = has_up ? (((jnz >> bit) & 1u) ? (((jneg >> bit) & 1u) ? -1 : 1) : 0) : 0;
+#pragma unroll
+            for (int mt = 0; mt < MT; ++mt) {
+                const int t = jsign * (((upw[mt] >> bit) & 1u) ? 1 : -1);
+                const double w1 = t > 0 ? eb : (t < 0 ? emb : 1.0);
+                const double w0 = t > 0 ? emb : (t < 0 ? eb : 1.0);
+                double nv[JT][2];
+                double ss = 0.0;
+#pragma unroll
+                for (int it = 0; it < JT; ++it)
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) {
+                        nv[it][e] = w0 * acc[mt][it][e] + w1 * acc[mt][JT + it][e];
+                        ss += nv[it][e] * nv[it][e];
+                    }
+                ss = quad_sum(ss);
+                const double sc = ss > 0.0 ? rsqrt(ss) : 0.0;    // PAPER.md:238 (any positive scale is equivalent)
+#pragma unroll
+                for (int it = 0; it < JT; ++it) {
+                    const double v0 = nv[it][0] * sc, v1 = nv[it][1] * sc;
+                    vf[mt][2 * it] = v0;
+                    vf[mt][2 * it + 1] = v1;
+                    double2* dst = reinterpret_cast<double2*>(
+                        renv + ((((size_t)col * SAMPLE_WARPS + warp) * MT + mt) * JT + it) * 64) + lane;
+                    *dst = make_double2(v0, v1);
+                }
+            }
+        }
+        // ============================================================ left sweep
+#pragma unroll
+        for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+            for (int kt = 0; kt < KT; ++kt) vf[mt][kt] = (kt == 0 && q == 0) ? 1.0 : 0.0;
+        cur_word = -1;
+        uint32_t neww = 0;          // owner lane: bits of the current word of the new row
+        uint32_t forcedw = 0;
+        double prod = 1.0;          // owner lane: running product of chosen probabilities
+        for (int col = 0; col < L; ++col, ++step) {
+            cp_async_wait<SAMPLE_STAGES - 2>();
+            __syncthreads();
+            issue_prefetch(step + SAMPLE_STAGES - 1);
+            const double* T = sT + (size_t)(step % SAMPLE_STAGES) * TSZ;   // tensor of site col
+            if ((col >> 5) != cur_word) {
+                cur_word = col >> 5;
+                if (has_up) {
+                    jneg = jd_neg[cur_word]; jnz = jd_nz[cur_word];
+#pragma unroll
+                    for (int mt = 0; mt < MT; ++mt) upw[mt] = sBits[chain_local[mt] * W + cur_word];
+                }
+                if (args.forced != nullptr && own_active)
+                    forcedw = args.forced[(own_out * L + r) * W + cur_word];
+                neww = 0;
+            }
+            double acc[MT][NT][2];
+#pragma unroll
+            for (int mt = 0; mt < MT; ++mt)
+#pragma unroll
+                for (int nt = 0; nt < NT; ++nt) { acc[mt][nt][0] = 0.0; acc[mt][nt][1] = 0.0; }
+            // t[chain][(a,j)] = sum_i Lenv[chain][i] T[i][a][j]
+#pragma unroll
+            for (int kt = 0; kt < KT; ++kt)
+#pragma unroll
+                for (int nt = 0; nt < NT; ++nt) {
+                    const double b = T[(kt * NT + nt) * 32 + lane];
+#pragma unroll
+                    for (int mt = 0; mt < MT; ++mt) dmma884(acc[mt][nt][0], acc[mt][nt][1], vf[mt][kt], b);
+                }
+            // rho_a = | t_a . R_col |
+            double rho0[MT], rho1[MT];
+#pragma unroll
+            for (int mt = 0; mt < MT; ++mt) {
+                double s0 = 0.0, s1 = 0.0;
+#pragma unroll
+                for (int jt = 0; jt < JT; ++jt) {
+                    const double2 rv = *(reinterpret_cast<const double2*>(
+                        renv + ((((size_t)col * SAMPLE_WARPS + warp) * MT + mt) * JT + jt) * 64) + lane);
+                    s0 += acc[mt][jt][0] * rv.x + acc[mt][jt][1] * rv.y;
+                    s1 += acc[mt][JT + jt][0] * rv.x + acc[mt][JT + jt][1] * rv.y;
+                }
+                rho0[mt] = fabs(quad_sum(s0));
+                rho1[mt] = fabs(quad_sum(s1));
+            }
+            // owner lane: conditional probability (Eq. 5), draw, log q
+            const int bit = col & 31;
+            const int jsign = has_up ? (((jnz >> bit) & 1u) ? (((jneg >> bit) & 1u) ? -1 : 1) : 0) : 0;
+            int a_sel = 0;
+            if (owner) {
+                double r0 = rho0[0], r1 = rho1[0];
+                uint32_t uw = upw[0];
+#pragma unroll
+                for (int mt = 1; mt < MT; ++mt) if (q == mt) { r0 = rho0[mt]; r1 = rho1[mt]; uw = upw[mt]; }
+                if (r0 == 0.0 || r1 == 0.0) {          // reading G10: count and clamp
+                    if (own_active) raise_flag(args.flags, FLAG_RHO_ZERO);
+                    if (r0 == 0.0) r0 = 2.2250738585072014e-308;
+                    if (r1 == 0.0) r1 = 2.2250738585072014e-308;
+                }
+                const int t = jsign * (((uw >> bit) & 1u) ? 1 : -1);
+                const double w1 = t > 0 ? eb : (t < 0 ? emb : 1.0);
+                const double w0 = t > 0 ? emb : (t < 0 ? eb : 1.0);
+                // sigma(log(r1/r0) + 2 beta J s_up) = r1 w1 / (r0 w0 + r1 w1)
+                const double f0 = r0 * w0, f1 = r1 * w1;
+                const double inv = 1.0 / (f0 + f1);
+                const double p1 = f1 * inv, p0 = f0 * inv;
+                const double u = philox_uniform((uint32_t)(r * L + col), ctr_samp, ctr_dis, TAG_SPIN,
+                                                args.seed_lo, args.seed_hi);
+                if (args.forced != nullptr) a_sel = (forcedw >> bit) & 1u;
+                else a_sel = u < p1;
+                if (own_active) {
+                    if (!(p1 >= 0.0 && p1 <= 1.0)) raise_flag(args.flags, FLAG_NONFINITE);
+                    if (fabs(u - p1) < 1e-9) raise_flag(args.flags, FLAG_NEAR_THRESHOLD);
+                    if (args.probs != nullptr) args.probs[(own_out * L + r) * L + col] = p1;
+                }
+                prod *= a_sel ? p1 : p0;
+                if (prod < 1e-200) { logq += log(prod); prod = 1.0; }
+                neww |= (uint32_t)a_sel << bit;
+                if (bit == 31 || col == L - 1) {
+                    if (own_active) args.cfg_bits[(own_out * L + r) * W + cur_word] = neww;
+                    // sBits of this word is no longer needed by the left sweep: overwrite for the next row
+                    sBits[own_local * W + cur_word] = neww;
+                }
+            }
+            // environment update with the sampled slice
+#pragma unroll
+            for (int mt = 0; mt < MT; ++mt) {
+                const int sel = __shfl_sync(0xffffffffu, a_sel, (lane & ~3) | mt);
+                double nv[JT][2];
+                double ss = 0.0;
+#pragma unroll
+                for (int jt = 0; jt < JT; ++jt)
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) {
+                        nv[jt][e] = sel ? acc[mt][JT + jt][e] : acc[mt][jt][e];
+                        ss += nv[jt][e] * nv[jt][e];
+                    }
+                ss = quad_sum(ss);
+                const double sc = ss > 0.0 ? rsqrt(ss) : 0.0;
+#pragma unroll
+                for (int jt = 0; jt < JT; ++jt) {
+                    vf[mt][2 * jt] = nv[jt][0] * sc;
+                    vf[mt][2 * jt + 1] = nv[jt][1] * sc;
+                }
+            }
+        }
+        if (owner) { logq += log(prod); prod = 1.0; }
+        __syncwarp();     // sBits written by owner lanes, read by the whole quad in the next row
+    }
+    if (own_active) args.logq[own_out] = logq;
+    cp_async_wait<0>();
+}
+
+}  // namespace tnmc

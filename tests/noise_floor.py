@@ -1,0 +1,57 @@
+"""Test helper: the oracle's own rounding-noise floor.
+
+The map row r+1 -> row r (MPO apply + truncation) can amplify a difference of
+rounding size by a large factor per row on frustrated instances (measured: x5..x10 per row at
+L=13, chi=5, beta=1.3), so two correct FP64 implementations that round differently (LAPACK in the
+oracle, Householder + one-sided Jacobi in the CUDA path) need not agree to the north_star's
+nominal 1e-10 / 1e-9 on such instances.  Both sides are NORM-WISE backward stable and no more
+(LAPACK's QR and SVD return the exact factors of A + dA with |dA| ~ p(n) eps |A|; small singular
+triplets carry absolute, not relative, accuracy).  The floor is therefore measured, per test case,
+by re-running the ORACLE's own steps with  A + 2^-52 * max|A| * N(0,1)  added to every tensor of
+the MPO x MPS product -- ONE rounding error's worth of norm-wise noise per row, where a QR + SVD
+sweep commits tens -- and comparing with the unperturbed oracle.  Parity
+tests use  tol = max(nominal, FLOOR_FACTOR * floor)  ("Tolerances").
+Only oracle/ is called here; nothing comes from the CUDA path.
+"""
+import numpy as np
+
+from oracle import bmps, sampler
+
+FLOOR_FACTOR = 20.0
+EPS = 2.0 ** -52
+
+
+def perturbed_cache(Jr, Jd, beta, chi, seed=12345, rel=EPS):
+    """oracle.bmps.build_cache with rounding-size norm-wise noise injected after every multiply."""
+    rng = np.random.default_rng(seed)
+    L = Jr.shape[0]
+    cache = [None] * L
+    logscale = np.zeros(L)
+    mps = bmps.bottom_mps(Jr, beta)
+    cache[L - 1] = mps
+    for row in range(L - 2, -1, -1):
+        mps = bmps.multiply(bmps.row_mpo(Jr, Jd, beta, row), mps)
+        mps = [A + rel * np.abs(A).max() * rng.standard_normal(A.shape) for A in mps]
+        ls, mps, _ = bmps.compress(mps, chi)
+        cache[row] = mps
+        logscale[row] = logscale[row + 1] + ls
+    return cache, logscale
+
+
+def state_floor(cache, cache_p):
+    """per row: max |Psihat - Psihat'| / max |Psihat| (needs L <= ~14)."""
+    out = []
+    for A, B in zip(cache, cache_p):
+        v, w = bmps.mps_to_vector(A), bmps.mps_to_vector(B)
+        out.append(np.abs(v - w).max() / np.abs(v).max())
+    return np.array(out)
+
+
+def logz_floor(cache, ls, cache_p, ls_p):
+    return abs(bmps.log_z(cache[0], ls[0])[0] - bmps.log_z(cache_p[0], ls_p[0])[0])
+
+
+def probs_floor(cache_p, Jd, beta, cfgs, probs, logq):
+    """max |p - p'| and max |log q - log q'| with the perturbed cache, teacher-forced on cfgs."""
+    _, lq, pr = sampler.sample(cache_p, Jd, beta, np.zeros(cfgs.shape), forced=cfgs)
+    return float(np.abs(pr - probs).max()), float(np.abs(lq - logq).max())
