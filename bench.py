@@ -1,0 +1,353 @@
+#!/usr/bin/env python
+"""bench.py -- accepted samples/s of the BatchTNMC hot path on synthetic +-J instances.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C2|C3|C4s|C5s] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path over one batch: tnmc_create (pack couplings) ->
+tnmc_build_envs -> tnmc_sample -> tnmc_energy -> tnmc_metropolis for every beta of the workload.
+`value` times the device-resident path (couplings already in HBM); `e2e` times tnmc_run_host with
+pinned HOST buffers (H2D of the couplings and D2H of configurations, E, log q, flags inside the
+timed region).  One JSON line on stdout (rank 0).  See DESIGN.md, "Measurement".
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from tnmc_workloads import CONFIGS, make_couplings  # noqa: E402
+
+# name -> (config key, n_dis, n_samples, ckpt_stride, note).  C2 (BASELINE.json configs[1]) is the
+# default; C3 is configs[2]; C4s / C5s are disorder x sample SLICES of configs[3] / configs[4] sized to
+# finish in minutes (the full configs are chunked runs of the same calls).
+WORKLOADS = {
+    "C1": ("C1", None, None, 0, "configs[0] 8x8 chi=16 exact"),
+    "C2": ("C2", None, None, 0, "configs[1] 32x32 chi=16 100x100 beta in {0.5,1,2}"),
+    "C3": ("C3", None, None, 0, "configs[2] 128x128 chi=32 256x256 FP64"),
+    "C4s": ("C4", 148, 200, 23, "configs[3] 512x512 chi=32, slice of 148 disorders x 200 samples, checkpoint stride 23"),
+    "C5s": ("C5", 74, 128, 32, "configs[4] 1024x1024 chi=32, slice of 74 disorders x 128 samples, checkpoint stride 32"),
+}
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="C2", choices=sorted(WORKLOADS))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def workload(name):
+    key, n_dis, n_s, ckpt, note = WORKLOADS[name]
+    c = dict(CONFIGS[key])
+    if n_dis:
+        c["n_dis"] = n_dis
+    if n_s:
+        c["n_samples"] = n_s
+    c["ckpt"] = ckpt
+    c["note"] = note
+    return c
+
+
+# ------------------------------------------------------------------------------------------------
+# clocks sampler (nvidia-smi, during the timed region)
+# ------------------------------------------------------------------------------------------------
+class Clocks:
+    Q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index):
+        self.index, self.rows, self.stop = index, [], threading.Event()
+        self.t = threading.Thread(target=self._run, daemon=True)
+
+    def _run(self):
+        while not self.stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits"],
+                                     capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([x.strip() for x in out.split(",")])
+            except Exception:
+                pass
+            self.stop.wait(0.2)
+
+    def __enter__(self):
+        self.t.start()
+        return self
+
+    def __exit__(self, *a):
+        self.stop.set()
+        self.t.join(timeout=6)
+
+    def summary(self):
+        sm = [float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(len(r) > 2 + i and r[2 + i].lower().startswith("active") for r in self.rows)]
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(self.rows)}
+
+
+# ------------------------------------------------------------------------------------------------
+# reference arm / cpu_baseline: the oracle as it stands, on the host cores
+# ------------------------------------------------------------------------------------------------
+def oracle_pass(c, beta, dis_ids, n_s):
+    """One pass of the oracle's whole path for the given disorders: returns accepted count."""
+    from oracle import bmps, exact, metropolis, philox, sampler
+    L, chi = c["L"], c["chi"]
+    accepted = 0
+    for d in dis_ids:
+        Jr, Jd = make_couplings(L, 1, c["inst_seed"], first_disorder=d)
+        Jr, Jd = Jr[0], Jd[0]
+        cache, ls = bmps.build_cache(Jr, Jd, beta, chi)
+        bmps.log_z(cache[0], ls[0])
+        u = np.empty((n_s, L, L))
+        samples = np.arange(n_s)
+        for r in range(L):
+            for col in range(L):
+                u[:, r, col] = philox.spin_uniforms(c["seed"], d, samples, r * L + col)
+        cfg, logq, _ = sampler.sample(cache, Jd, beta, u)
+        E = exact.energy(cfg, Jr, Jd)
+        um = philox.metropolis_uniforms(c["seed"], d, samples)
+        _, n_acc, *_ = metropolis.metropolis_scan(E, logq, beta, um)
+        accepted += n_acc
+    return accepted
+
+
+def oracle_sample_sizes(c, budget_s):
+    """(n disorders, n samples) of a bounded sample costing roughly budget_s seconds of one core."""
+    L, chi = c["L"], c["chi"]
+    per_dis = 0.35 * (L / 32.0) ** 2 * (chi / 16.0) ** 3            # build, calibrated at L=32, chi=16
+    per_chain = 0.007 * (L / 32.0) ** 2 * (chi / 16.0) ** 2          # sampler + uniforms per sample
+    n_s = min(c["n_samples"], 100)
+    n_d = int(max(1, min(c["n_dis"], budget_s / (len(c["betas"]) * (per_dis + n_s * per_chain)))))
+    return n_d, n_s
+
+
+def run_oracle(c, n_d, n_s):
+    t0 = time.perf_counter()
+    acc = 0
+    for beta in c["betas"]:
+        acc += oracle_pass(c, beta, range(n_d), n_s)
+    dt = time.perf_counter() - t0
+    return acc, dt
+
+
+def threads_used():
+    try:
+        from threadpoolctl import threadpool_info
+        return max([p.get("num_threads", 1) for p in threadpool_info()] + [1])
+    except Exception:
+        return os.cpu_count() or 1
+
+
+def main_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    c = workload(args.workload)
+    n_d, n_s = oracle_sample_sizes(c, 6.0)
+    for _ in range(min(args.warmup, 1)):
+        run_oracle(c, 1, min(n_s, 8))
+    tot_acc, tot_t = 0, 0.0
+    for _ in range(args.steps):
+        acc, dt = run_oracle(c, n_d, n_s)
+        tot_acc += acc
+        tot_t += dt
+    val = tot_acc / tot_t
+    sample = f"{n_d} disorders x {n_s} samples x {len(c['betas'])} betas of {args.workload} per step (whole path: build, sample, energy, Metropolis)"
+    line = {"impl": "reference", "metric": "accepted samples/s", "value": val, "unit": "samples/s", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": args.workload, "L": c["L"], "chi": c["chi"], "betas": list(c["betas"]), "note": c["note"]},
+            "cpu_baseline": {"value": val, "unit": "samples/s", "cores": threads_used(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": "samples/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------
+# our arm
+# ------------------------------------------------------------------------------------------------
+def main_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2509_19006_b200 import model, tnmc
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the hot path has no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    c = workload(args.workload)
+    L, chi, n_dis, n_s, ckpt = c["L"], c["chi"], c["n_dis"], c["n_samples"], c["ckpt"]
+    P = model.pad_chi(chi)
+    betas = list(c["betas"])
+    # weak scaling: every rank owns its own n_dis disorders (global indices rank*n_dis ...); no collective on the data path
+    first = rank * n_dis
+    Jr_np, Jd_np = make_couplings(L, n_dis, c["inst_seed"], first_disorder=first)
+    Jr_h, Jd_h = torch.from_numpy(Jr_np).pin_memory(), torch.from_numpy(Jd_np).pin_memory()
+    Jr, Jd = Jr_h.to(dev), Jd_h.to(dev)
+    need = tnmc.tnmc_workspace_bytes(L, chi, n_dis, n_s, ckpt_stride=ckpt)
+    need_h = tnmc.tnmc_run_host_workspace_bytes(L, chi, n_dis, n_s, ckpt_stride=ckpt)
+    ws = torch.empty(max(need, need_h), dtype=torch.uint8, device=dev)
+    W = tnmc.words(L)
+    bits = torch.empty((n_dis, n_s, L, W), dtype=torch.int32, device=dev)
+    logq = torch.empty((n_dis, n_s), dtype=torch.float64, device=dev)
+    E = torch.empty((n_dis, n_s), dtype=torch.int32, device=dev)
+    logZ = torch.empty(n_dis, dtype=torch.float64, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
+    stream = torch.cuda.current_stream()
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+
+    def step(timed):
+        """one pass over the batch; returns (accepted, launches, phase ms dict)"""
+        acc, launches = 0, 0
+        ph = {"build": 0.0, "sample": 0.0, "energy": 0.0, "metropolis": 0.0}
+        evs = []
+        for beta in betas:
+            ctx = tnmc.Context(L, chi, beta, Jr, Jd, n_s, first_disorder=first, ckpt_stride=ckpt, workspace=ws)
+            e = [ev() for _ in range(5)]
+            e[0].record(stream); ctx.tnmc_build_envs(logZ)
+            e[1].record(stream); ctx.tnmc_sample(n_s, c["seed"], cfg_bits=bits, logq=logq)
+            e[2].record(stream); ctx.tnmc_energy(bits, E=E)
+            e[3].record(stream); _, n_acc, _, _ = ctx.tnmc_metropolis(E, logq, c["seed"])
+            e[4].record(stream)
+            evs.append((e, n_acc, ctx))
+        torch.cuda.synchronize()
+        for e, n_acc, ctx in evs:
+            acc += int(n_acc.sum().item())
+            launches += ctx.tnmc_launch_count()
+            for i, k in enumerate(ph):
+                ph[k] += e[i].elapsed_time(e[i + 1])
+            ctx.close()
+        return acc, launches, ph
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+
+    for _ in range(max(args.warmup, 3)):
+        step(False)
+    phases = {"build": 0.0, "sample": 0.0, "energy": 0.0, "metropolis": 0.0}
+    tot_ms, tot_acc, tot_launch = 0.0, 0, 0
+    with Clocks(local_rank) as clk:
+        for _ in range(args.steps):
+            flush.zero_()                                   # L2 flush between timed iterations
+            barrier()
+            e0, e1 = ev(), ev()
+            e0.record(stream)
+            acc, launches, ph = step(True)
+            e1.record(stream)
+            barrier()
+            tot_ms += e0.elapsed_time(e1)
+            tot_acc += acc
+            tot_launch += launches
+            for k in phases:
+                phases[k] += ph[k]
+    t = torch.tensor([tot_ms], dtype=torch.float64, device=dev)
+    a = torch.tensor([float(tot_acc)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(a, op=dist.ReduceOp.SUM)
+    ms_total, acc_total = t.item(), a.item()
+    value = acc_total / (ms_total * 1e-3)
+
+    # ---- end to end: host buffers through tnmc_run_host
+    e2e = None
+    if not args.no_e2e:
+        outs = None
+        for _ in range(2):
+            for beta in betas:
+                outs = tnmc.tnmc_run_host(L, chi, beta, Jr_h, Jd_h, n_s, c["seed"], ws, first_disorder=first, ckpt_stride=ckpt, out=outs)
+        e_acc, t0 = 0, None
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            for beta in betas:
+                outs = tnmc.tnmc_run_host(L, chi, beta, Jr_h, Jd_h, n_s, c["seed"], ws, first_disorder=first, ckpt_stride=ckpt, out=outs)
+                e_acc += int(outs["n_accepted"].sum().item())
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        te = torch.tensor([dt], dtype=torch.float64, device=dev)
+        ae = torch.tensor([float(e_acc)], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+            dist.all_reduce(ae, op=dist.ReduceOp.SUM)
+        h2d = len(betas) * (Jr_h.numel() + Jd_h.numel())
+        d2h = len(betas) * sum(v.numel() * v.element_size() for v in outs.values() if v is not None)
+        e2e = {"value": ae.item() / te.item(), "unit": "samples/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h}
+
+    if rank == 0:
+        nb = len(betas) * args.steps
+        build_ms = phases["build"] / nb                      # average duration of one tnmc_build_envs (one build_rows_kernel launch)
+        sample_ms = phases["sample"] / nb
+        build_flops = model.build_flops_per_disorder(L, chi) * n_dis * (2.0 if ckpt else 1.0)
+        peak_dmma = tnmc.tnmc_fp64_peak_tflops(1)
+        peak_dfma = tnmc.tnmc_fp64_peak_tflops(0)
+        peaks = {}
+        try:
+            peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        except Exception:
+            pass
+        hbm_peak = peaks.get("hbm_gbs", 6650.0)
+        samp_flops = model.sample_flops_per_chain_site(P) * n_dis * n_s * L * L
+        samp_bytes = model.sample_bytes_per_chain_site(P) * n_dis * n_s * L * L
+        dominant = "build_rows_kernel" if phases["build"] >= phases["sample"] else "sample_rows_kernel"
+        if dominant == "build_rows_kernel":
+            ach = build_flops / (build_ms * 1e-3) / 1e12
+            roof = {"bound": "alu", "kernel": dominant, "achieved": ach, "peak": peak_dfma, "unit": "TFLOP/s", "frac": ach / peak_dfma,
+                    "traffic": None, "peak_source": "FP64 DFMA rate measured live by tnmc_fp64_peak_tflops(0) on this GPU",
+                    "algorithmic_flops_per_launch": build_flops}
+        else:
+            ach = samp_flops / (sample_ms * 1e-3) / 1e12
+            roof = {"bound": "tensor", "kernel": dominant, "achieved": ach, "peak": peak_dmma, "unit": "TFLOP/s", "frac": ach / peak_dmma,
+                    "traffic": None, "peak_source": "FP64 DMMA (mma.sync.m8n8k4.f64) rate measured live by tnmc_fp64_peak_tflops(1)",
+                    "algorithmic_flops_per_launch": samp_flops}
+        roof["other_kernels"] = {
+            "sample_rows_kernel": {"ms": sample_ms, "tflops": samp_flops / (sample_ms * 1e-3) / 1e12, "frac_dmma_peak": samp_flops / (sample_ms * 1e-3) / 1e12 / peak_dmma,
+                                   "hbm_gbs": samp_bytes / (sample_ms * 1e-3) / 1e9, "frac_hbm_peak": samp_bytes / (sample_ms * 1e-3) / 1e9 / hbm_peak},
+            "build_rows_kernel": {"ms": build_ms, "tflops": build_flops / (build_ms * 1e-3) / 1e12, "frac_dfma_peak": build_flops / (build_ms * 1e-3) / 1e12 / peak_dfma},
+            "fp64_peaks_tflops": {"dfma": peak_dfma, "dmma": peak_dmma, "hbm_gbs": hbm_peak},
+        }
+        cpu = None
+        if not args.no_cpu_baseline and world == 1:
+            n_d, n_so = oracle_sample_sizes(c, 15.0)
+            acc_o, dt_o = run_oracle(c, n_d, n_so)
+            cpu = {"value": acc_o / dt_o, "unit": "samples/s", "cores": threads_used(), "kind": "oracle", "seconds": dt_o,
+                   "sample": f"{n_d} disorders x {n_so} samples x {len(betas)} betas of {args.workload} (whole path)"}
+        line = {"metric": "accepted samples/s", "value": value, "unit": "samples/s", "n_gpus": world, "steps": args.steps,
+                "warmup": max(args.warmup, 3), "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": {"workload": args.workload, "note": c["note"], "L": L, "chi": chi, "betas": betas, "n_dis_per_gpu": n_dis,
+                           "n_samples": n_s, "ckpt_stride": ckpt, "parallelism": f"dp{world} (disorders sharded, no collective)",
+                           "l2": "flushed (256 MiB memset) between timed steps; env stack > L2"},
+                "proposals_per_s": len(betas) * args.steps * n_dis * n_s * world / (ms_total * 1e-3),
+                "p_acc": acc_total / (len(betas) * args.steps * n_dis * (n_s - 1) * world),
+                "phase_ms_per_step": {k: v / args.steps for k, v in phases.items()},
+                "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": tot_launch, "clocks": clk.summary()}
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    a = parse()
+    sys.exit(main_reference(a) if a.impl == "reference" else main_ours(a))

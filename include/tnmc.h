@@ -179,6 +179,12 @@ tnmc_status tnmc_get_flags(tnmc_ctx* ctx, uint64_t* host_flags_out);
 tnmc_status tnmc_get_env_row(tnmc_ctx* ctx, int disorder, int row, double* out,
                              double* logscale_out);
 
+/* Roofline denominator probe: runs a register-resident FP64 microbenchmark on the current device
+ * (148 x 2 CTAs of 256 threads, 8 independent chains per thread) for a few milliseconds and
+ * returns the sustained rate in TFLOP/s: which = 0 -> scalar DFMA, which = 1 -> mma.sync.m8n8k4.f64
+ * (DMMA).  scratch [dev] >= 1 MiB.  Synchronises.  Returns a negative value on a CUDA error. */
+double tnmc_fp64_peak_tflops(int which, void* scratch, void* cuda_stream);
+
 /* Number of kernels this context has launched so far (bench.py's gpu_launches). */
 uint64_t tnmc_launch_count(const tnmc_ctx* ctx);
 

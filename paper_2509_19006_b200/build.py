@@ -7,8 +7,13 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtnmc.so")
 SOURCES = ["tnmc.cu"]
-HEADERS = ["tnmc_common.cuh", "tnmc_build.cuh", "tnmc_sample.cuh", "tnmc_energy.cuh", "tnmc_ctx.cuh",
-           os.path.join("..", "..", "include", "tnmc.h")]
+
+
+def _deps():
+    """every file the library is compiled from: csrc/*.cu, csrc/*.cuh and include/tnmc.h"""
+    files = [os.path.join(CSRC, f) for f in sorted(os.listdir(CSRC)) if f.endswith((".cu", ".cuh", ".h"))]
+    files.append(os.path.join(HERE, "..", "include", "tnmc.h"))
+    return files
 
 
 def _nvcc():
@@ -22,8 +27,7 @@ def needs_build():
     if not os.path.exists(LIB):
         return True
     t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, f) for f in SOURCES + HEADERS]
-    return any(os.path.getmtime(d) > t for d in deps)
+    return any(os.path.getmtime(d) > t for d in _deps())
 
 
 def build(force=False, verbose=False):

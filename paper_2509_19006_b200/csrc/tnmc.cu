@@ -371,3 +371,65 @@ extern "C" tnmc_status tnmc_run_host(int L, int chi, double beta, int n_dis, int
     if (e != cudaSuccess) return done(cuda_fail(ctx, e, "tnmc_run_host: copy back"));
     return done(TNMC_OK);
 }
+
+// ---------------------------------------------------------------------------------------------
+// FP64 peak probe (roofline denominator for bench.py)
+// ---------------------------------------------------------------------------------------------
+namespace {
+__global__ void __launch_bounds__(256) peak_dfma_kernel(double* out, int iters) {
+    double a0 = 1.0 + threadIdx.x * 1e-9, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
+    const double b = 1.0000001, c = 1e-9;
+    for (int i = 0; i < iters; ++i) {
+        a0 = fma(a0, b, c); a1 = fma(a1, b, c); a2 = fma(a2, b, c); a3 = fma(a3, b, c);
+        a4 = fma(a4, b, c); a5 = fma(a5, b, c); a6 = fma(a6, b, c); a7 = fma(a7, b, c);
+    }
+    out[blockIdx.x * blockDim.x + threadIdx.x] = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+}
+__global__ void __launch_bounds__(256) peak_dmma_kernel(double* out, int iters) {
+    double c[8][2];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { c[i][0] = 0.0; c[i][1] = 0.0; }
+    const double a = 1.0 + threadIdx.x * 1e-9, b = 1e-9 * threadIdx.x;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) dmma884(c[j][0], c[j][1], a, b);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += c[i][0] + c[i][1];
+    out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+}  // namespace
+
+extern "C" double tnmc_fp64_peak_tflops(int which, void* scratch, void* cuda_stream) {
+    cudaStream_t s = reinterpret_cast<cudaStream_t>(cuda_stream);
+    double* out = reinterpret_cast<double*>(scratch);
+    const int blocks = 148 * 2, threads = 256, iters = 20000;
+    cudaEvent_t e0, e1;
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return -1.0;
+    float best = 1e30f;
+    for (int rep = 0; rep < 3; ++rep) {
+        cudaEventRecord(e0, s);
+        if (which == 0) peak_dfma_kernel<<<blocks, threads, 0, s>>>(out, iters);
+        else peak_dmma_kernel<<<blocks, threads, 0, s>>>(out, iters);
+        cudaEventRecord(e1, s);
+        if (cudaEventSynchronize(e1) != cudaSuccess) { best = -1.0f; break; }
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (rep > 0 && ms < best) best = ms;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    if (best <= 0.f) return -1.0;
+    const double flops = which == 0 ? 2.0 * 8 * iters * (double)blocks * threads
+                                    : 2.0 * 256 * 8 * iters * (double)blocks * (threads / 32);
+    return flops / (best * 1e-3) / 1e12;
+}
+
+#ifdef TNMC_PROFILE
+// debug build only: per-phase clock64 totals of CTA 0 of build_rows_kernel
+extern "C" void tnmc_debug_build_profile(unsigned long long* out16, int reset) {
+    cudaDeviceSynchronize();
+    cudaMemcpyFromSymbol(out16, tnmc::g_build_prof, sizeof(unsigned long long) * 256);
+    if (reset) { unsigned long long z[256] = {0}; cudaMemcpyToSymbol(tnmc::g_build_prof, z, sizeof(z)); }
+}
+#endif

@@ -10,10 +10,21 @@
 // C_a = sum_m B_d[a,m] A[i,m,k], so the carried R of the QR sweep only ever meets C_a.
 #pragma once
 #include "tnmc_common.cuh"
+#include "tnmc_linalg.cuh"
 
 namespace tnmc {
 
 constexpr int BUILD_THREADS = 256;
+
+#ifdef TNMC_PROFILE
+#define PROF_DECL long long prof_t0 = clock64();
+#define PROF(slot) do { if (blockIdx.x == 0 && threadIdx.x == 0) { const long long t_ = clock64(); atomicAdd(&g_build_prof[slot], (unsigned long long)(t_ - prof_t0)); prof_t0 = t_; } } while (0)
+#define PROF_ADD(slot, v) do { if (blockIdx.x == 0 && threadIdx.x == 0) atomicAdd(&g_build_prof[slot], (unsigned long long)(v)); } while (0)
+#else
+#define PROF_DECL
+#define PROF(slot)
+#define PROF_ADD(slot, v)
+#endif
 
 struct BuildArgs {
     JView J;
@@ -48,175 +59,6 @@ struct BuildCfg {
     static size_t smem_bytes(int L) { return sizeof(double) * N_DBL + sizeof(int) * (L + 2 + 2 * D); }
 };
 
-// block-wide sum of one double per thread; result valid in all threads. scratch: >= 32 doubles
-__device__ __forceinline__ double block_sum(double v, double* scratch) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
-    __syncthreads();
-    if (l == 0) scratch[w] = v;
-    __syncthreads();
-    double t = 0.0;
-    const int nw = blockDim.x >> 5;
-    for (int i = 0; i < nw; ++i) t += scratch[i];
-    return t;
-}
-
-// Householder QR of the m x n column-major matrix X (leading dim ld) in shared memory.
-// On return the upper trapezoid holds R, the reflector vectors (v_j, unit diagonal implied) sit
-// below the diagonal, tau[j] their scalars; kk = min(m,n) reflectors.
-__device__ void householder_qr(double* X, int ld, int m, int n, double* tau) {
-    const int kk = m < n ? m : n;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
-    for (int j = 0; j < kk; ++j) {
-        double* colj = X + (size_t)j * ld;
-        if (warp == 0) {
-            double ss = 0.0;
-            for (int i = j + 1 + lane; i < m; i += 32) { const double v = colj[i]; ss += v * v; }
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
-            const double alpha = colj[j];
-            double t = 0.0, scale = 0.0, bet = alpha;
-            if (ss != 0.0) {
-                const double nrm = sqrt(alpha * alpha + ss);
-                bet = alpha >= 0.0 ? -nrm : nrm;
-                t = (bet - alpha) / bet;
-                scale = 1.0 / (alpha - bet);
-            }
-            __syncwarp();
-            for (int i = j + 1 + lane; i < m; i += 32) colj[i] *= scale;
-            if (lane == 0) { colj[j] = bet; tau[j] = t; }
-        }
-        __syncthreads();
-        const double t = tau[j];
-        if (t != 0.0) {
-            for (int jj = j + 1 + warp; jj < n; jj += nwarps) {
-                double* col = X + (size_t)jj * ld;
-                double w = 0.0;
-                for (int i = j + 1 + lane; i < m; i += 32) w += colj[i] * col[i];
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) w += __shfl_xor_sync(0xffffffffu, w, o);
-                w += col[j];
-                w *= t;
-                __syncwarp();
-                for (int i = j + 1 + lane; i < m; i += 32) col[i] -= w * colj[i];
-                if (lane == 0) col[j] -= w;
-            }
-        }
-        __syncthreads();
-    }
-}
-
-// Overwrite the reflectors with the explicit thin Q (m x kk), in place (LAPACK dorg2r order).
-__device__ void householder_form_q(double* X, int ld, int m, int kk, const double* tau) {
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
-    for (int j = kk - 1; j >= 0; --j) {
-        double* colj = X + (size_t)j * ld;
-        const double t = tau[j];
-        if (t != 0.0) {
-            for (int jj = j + 1 + warp; jj < kk; jj += nwarps) {
-                double* col = X + (size_t)jj * ld;
-                double w = 0.0;
-                for (int i = j + 1 + lane; i < m; i += 32) w += colj[i] * col[i];
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) w += __shfl_xor_sync(0xffffffffu, w, o);
-                // row j of the trailing block is e_j-free here: Q[j][jj] = 0 before H_j is applied
-                w *= t;
-                __syncwarp();
-                for (int i = j + 1 + lane; i < m; i += 32) col[i] -= w * colj[i];
-                if (lane == 0) col[j] = -w;
-            }
-        } else {
-            for (int jj = j + 1 + warp; jj < kk; jj += nwarps)
-                if (lane == 0) X[(size_t)jj * ld + j] = 0.0;
-        }
-        __syncthreads();
-        for (int i = threadIdx.x; i < m; i += blockDim.x) {
-            double v;
-            if (i < j) v = 0.0;
-            else if (i == j) v = 1.0 - t;
-            else v = -t * colj[i];
-            colj[i] = v;
-        }
-        __syncthreads();
-    }
-}
-
-// One-sided (Hestenes) Jacobi on the ROWS of the n x nc row-major matrix M (row length ld):
-// plane rotations from the left until all rows are mutually orthogonal, so that row x ends as
-// sigma_x * v_x^T (M = U Sigma V^T).  n must be even (callers pad with a zero row).
-// Eight threads cooperate on one row pair; pairs follow the round-robin (circle) schedule.
-// Returns the number of sweeps done (all threads).
-// Rows whose squared norm is <= thr2 (numerically zero against |M|_F) are left alone: when M has
-// more rows than its rank they only carry rounding noise, and chasing their orthogonality would
-// grind them down to denormals without ever meeting the relative criterion.
-__device__ int jacobi_rows(double* M, int ld, int n, int nc, double thr2, unsigned long long* flags) {
-    const int grp = threadIdx.x >> 3, t8 = threadIdx.x & 7;
-    const int npairs = n >> 1;
-    const unsigned gmask = 0xffu << ((threadIdx.x & 31) & ~7);
-    // A pair is rotated whenever its cosine exceeds one rounding error; the sweeps stop after the
-    // first one in which every cosine met was below 1e-8: cyclic Jacobi converges quadratically, so
-    // the rotations of that last sweep leave the rows orthogonal to rounding level (the accuracy
-    // LAPACK's SVD gives the oracle).  A looser stop (cosines ~1e-14) was measurably not enough:
-    // the row-to-row map amplifies such errors by up to ~1e6 ("Tolerances").
-    const double rot2 = 4.930380657631324e-32;     // (2^-52)^2
-    const double big2 = 1e-16;                     // (1e-8)^2
-    int sweep = 0;
-    for (; sweep < 60; ++sweep) {
-        int any = 0;
-        for (int round = 0; round < n - 1; ++round) {
-            int rotated = 0;
-            for (int p = grp; p < npairs; p += (blockDim.x >> 3)) {
-                int r1, r2;
-                if (p == 0) { r1 = n - 1; r2 = round; }
-                else {
-                    r1 = (round + p) % (n - 1);
-                    r2 = (round - p + (n - 1)) % (n - 1);
-                }
-                if (r1 > r2) { const int t = r1; r1 = r2; r2 = t; }
-                double* x = M + (size_t)r1 * ld;
-                double* y = M + (size_t)r2 * ld;
-                double a = 0.0, b = 0.0, g = 0.0;
-                for (int c = 2 * t8; c < nc; c += 16) {
-                    const double x0 = x[c], y0 = y[c];
-                    a += x0 * x0; b += y0 * y0; g += x0 * y0;
-                    if (c + 1 < nc) {
-                        const double x1 = x[c + 1], y1 = y[c + 1];
-                        a += x1 * x1; b += y1 * y1; g += x1 * y1;
-                    }
-                }
-#pragma unroll
-                for (int o = 4; o > 0; o >>= 1) {
-                    a += __shfl_xor_sync(gmask, a, o);
-                    b += __shfl_xor_sync(gmask, b, o);
-                    g += __shfl_xor_sync(gmask, g, o);
-                }
-                if (a > thr2 && b > thr2 && g * g > rot2 * (a * b)) {
-                    rotated |= g * g > big2 * (a * b);
-                    const double zeta = (b - a) / (2.0 * g);
-                    const double tt = (zeta >= 0.0 ? 1.0 : -1.0) / (fabs(zeta) + sqrt(1.0 + zeta * zeta));
-                    const double cs = 1.0 / sqrt(1.0 + tt * tt);
-                    const double sn = cs * tt;
-                    for (int c = 2 * t8; c < nc; c += 16) {
-                        const double x0 = x[c], y0 = y[c];
-                        x[c] = cs * x0 - sn * y0;
-                        y[c] = sn * x0 + cs * y0;
-                        if (c + 1 < nc) {
-                            const double x1 = x[c + 1], y1 = y[c + 1];
-                            x[c + 1] = cs * x1 - sn * y1;
-                            y[c + 1] = sn * x1 + cs * y1;
-                        }
-                    }
-                }
-            }
-            any |= __syncthreads_or(rotated);
-        }
-        if (!any) break;
-    }
-    if (sweep >= 60 && threadIdx.x == 0) raise_flag(flags, FLAG_JACOBI_LIMIT);
-    return sweep;
-}
-
 template <int P>
 __global__ void __launch_bounds__(BUILD_THREADS, 1) build_rows_kernel(const BuildArgs args) {
     using Cfg = BuildCfg<P>;
@@ -240,6 +82,7 @@ __global__ void __launch_bounds__(BUILD_THREADS, 1) build_rows_kernel(const Buil
     double* qbuf_d = args.qbuf + (size_t)d * (size_t)L * Cfg::QSZ;
     double* ls_d = args.logscale + (size_t)d * L;
 
+    PROF_DECL
     for (int r = args.row_hi - 1; r >= args.row_lo; --r) {
         const double* env_in = env_d + (size_t)args.slot_of_row[r + 1] * L * TSZ;
         double* env_out = env_d + (size_t)args.slot_of_row[r] * L * TSZ;
@@ -290,7 +133,9 @@ __global__ void __launch_bounds__(BUILD_THREADS, 1) build_rows_kernel(const Buil
                 __syncthreads();
                 break;
             }
+            PROF(0);
             householder_qr(sX, LDX, m, n, sS);
+            PROF(1);
             const int kk = m < n ? m : n;
             // R -> carried R/|R|_F for the next site; logscale += log |R|_F
             double ss = 0.0;
@@ -310,7 +155,9 @@ __global__ void __launch_bounds__(BUILD_THREADS, 1) build_rows_kernel(const Buil
             }
             if (tid == 0) sq[c + 1] = kk;
             __syncthreads();
+            PROF(2);
             householder_form_q(sX, LDX, m, kk, sS);
+            PROF(3);
             for (int t = tid; t < m * kk; t += BUILD_THREADS) {
                 const int row = t % m, col = t / m;
                 Qout[row + (size_t)col * LDX] = sX[row + (size_t)col * LDX];
@@ -379,7 +226,10 @@ __global__ void __launch_bounds__(BUILD_THREADS, 1) build_rows_kernel(const Buil
             }
             fro2 = block_sum(fro2, sRed);
             const double thr2 = fro2 * 1e-30;      // sigma <= 1e-15 |M|_F: below the numerical rank
-            jacobi_rows(sM, LDM, nrow, nc, thr2, args.flags);
+            PROF(4);
+            const int nsw = jacobi_rows(sM, LDM, nrow, nc, fro2, thr2, sS, args.flags);
+            PROF(5);
+            PROF_ADD(8, nsw); PROF_ADD(9, 1);
             // singular values = row norms
             {
                 const int grp = tid >> 3, t8 = tid & 7;
@@ -432,6 +282,7 @@ __global__ void __launch_bounds__(BUILD_THREADS, 1) build_rows_kernel(const Buil
             __syncthreads();
             { double* t = sPc; sPc = sPn; sPn = t; }
             kprev = k;
+            PROF(6);
         }
         if (tid == 0) ls_d[r] = ls_d[r + 1] + logs;
         __syncthreads();

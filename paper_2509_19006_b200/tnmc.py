@@ -49,6 +49,8 @@ def _load():
     lib.tnmc_get_flags.argtypes = [vp, vp]
     lib.tnmc_get_env_row.restype = i32
     lib.tnmc_get_env_row.argtypes = [vp, i32, i32, vp, vp]
+    lib.tnmc_fp64_peak_tflops.restype = dbl
+    lib.tnmc_fp64_peak_tflops.argtypes = [i32, vp, vp]
     lib.tnmc_launch_count.restype = u64
     lib.tnmc_launch_count.argtypes = [vp]
     lib.tnmc_last_error.restype = C.c_char_p
@@ -218,3 +220,13 @@ def tnmc_run_host(L, chi, beta, Jr_host, Jd_host, n_samples, seed, workspace, fi
                            hp(out["logZ"], torch.float64), hp(out["n_accepted"], torch.int64))
     _check(st)
     return out
+
+
+def tnmc_fp64_peak_tflops(which, scratch=None):
+    """Live FP64 roofline probe: which=0 scalar DFMA, which=1 DMMA (mma.sync.m8n8k4.f64)."""
+    if scratch is None:
+        scratch = torch.empty(1 << 20, dtype=torch.uint8, device="cuda")
+    v = float(lib.tnmc_fp64_peak_tflops(which, _ptr(scratch, torch.uint8), _stream()))
+    if v <= 0:
+        raise TnmcError(TNMC_ECUDA, "tnmc_fp64_peak_tflops failed")
+    return v
