@@ -50,8 +50,9 @@ struct BuildCfg {
     static constexpr int QSZ = LDX * D;       // doubles per site of the Q scratch
     // shared-memory carve-up (doubles)
     static constexpr int X_OFF = 0;                   // LDX*D : QR operand / Q_c / staging
-    static constexpr int R_OFF = X_OFF + LDX * D;     // D*D   : carried R [x][lambda] / Jacobi operand M
-    static constexpr int A_OFF = R_OFF + D * D;       // TSZ   : lower-row site tensor (fragment order) / Pc
+    static constexpr int R_OFF = X_OFF + LDX * D;     // D*LDC : carried R [x][lambda] (ld D) / column-major M for QRCP (ld LDC)
+    static constexpr int LDC = D + 1;         // leading dim of the column-major copy of M that QRCP works on
+    static constexpr int A_OFF = R_OFF + D * LDC;     // TSZ   : lower-row site tensor (fragment order) / Pc
     static constexpr int C_OFF = A_OFF + TSZ;         // TSZ   : C_a[i][k] / Pc_new
     static constexpr int M0_OFF = C_OFF + TSZ;        // D*LDM : copy of M before rotation
     static constexpr int S_OFF = M0_OFF + D * LDM;    // 2*D + 8 : tau / sigma / scalars
@@ -62,7 +63,7 @@ struct BuildCfg {
 template <int P>
 __global__ void __launch_bounds__(BUILD_THREADS, 1) build_rows_kernel(const BuildArgs args) {
     using Cfg = BuildCfg<P>;
-    constexpr int D = Cfg::D, LDX = Cfg::LDX, LDM = Cfg::LDM, LDV = Cfg::LDV, TSZ = Cfg::TSZ;
+    constexpr int D = Cfg::D, LDX = Cfg::LDX, LDM = Cfg::LDM, LDV = Cfg::LDV, TSZ = Cfg::TSZ, LDC = Cfg::LDC;
     extern __shared__ __align__(16) double smem[];
     double* sX = smem + Cfg::X_OFF;
     double* sR = smem + Cfg::R_OFF;
@@ -134,7 +135,7 @@ __global__ void __launch_bounds__(BUILD_THREADS, 1) build_rows_kernel(const Buil
                 break;
             }
             PROF(0);
-            householder_qr(sX, LDX, m, n, sS);
+            householder_qr<P>(sX, LDX, m, n, sS);
             PROF(1);
             const int kk = m < n ? m : n;
             // R -> carried R/|R|_F for the next site; logscale += log |R|_F
@@ -156,7 +157,7 @@ __global__ void __launch_bounds__(BUILD_THREADS, 1) build_rows_kernel(const Buil
             if (tid == 0) sq[c + 1] = kk;
             __syncthreads();
             PROF(2);
-            householder_form_q(sX, LDX, m, kk, sS);
+            householder_form_q<P>(sX, LDX, m, kk, sS);
             PROF(3);
             for (int t = tid; t < m * kk; t += BUILD_THREADS) {
                 const int row = t % m, col = t / m;
@@ -166,7 +167,9 @@ __global__ void __launch_bounds__(BUILD_THREADS, 1) build_rows_kernel(const Buil
         }
 
         // ------------------------------------------------------------------ SVD sweep, right -> left
-        double* sM = sR;          // Jacobi operand, row-major [x][a*kprev + y], ld = LDM
+        double* sMc = sR;         // M, column-major [x + col*LDC]: QRCP operand
+        double* sM = sX;          // Jacobi operand (rows of R), row-major, ld = LDM; lives in sX once Q_c is consumed
+        int* sperm = spos + D;    // column permutation of the QRCP
         double* sPc = sA;         // carried M V_k of the site to the right: [z][y], ld = P
         double* sPn = sC;
         int kprev = 1;
@@ -187,18 +190,18 @@ __global__ void __launch_bounds__(BUILD_THREADS, 1) build_rows_kernel(const Buil
                 const double* Xrow = sX + (2 * x + a);
                 double acc = 0.0;
                 for (int z = 0; z < qr; ++z) acc += Xrow[(size_t)z * LDX] * sPc[z * P + y];
-                sM[(size_t)x * LDM + a * kprev + y] = acc;
+                sMc[x + (size_t)(a * kprev + y) * LDC] = acc;
                 sM0[(size_t)x * LDM + a * kprev + y] = acc;
             }
             __syncthreads();
-            double* stage = sX;                 // TSZ doubles: output tensor in fragment order
-            double* sV = sX + TSZ;              // [y'][col], ld = LDV: selected right singular vectors
+            double* stage = sX + D * LDM;       // TSZ doubles: output tensor in fragment order
+            double* sV = stage + TSZ;           // [y'][col], ld = LDV: selected right singular vectors
             for (int t = tid; t < TSZ; t += BUILD_THREADS) stage[t] = 0.0;
             double* Aout = env_out + (size_t)c * TSZ;
             if (c == 0) {
                 // P-C2 step 3: A_0 (1,2,k_1) = Q_0 Pc; divide by its norm, add log to logscale
                 double ss = 0.0;
-                for (int t = tid; t < nc; t += BUILD_THREADS) ss += sM[t] * sM[t];
+                for (int t = tid; t < nc; t += BUILD_THREADS) ss += sM0[t] * sM0[t];
                 ss = block_sum(ss, sRed);
                 const double s = sqrt(ss);
                 if (!(s > 0.0) || !isfinite(s)) { if (tid == 0) raise_flag(args.flags, FLAG_NONFINITE); }
@@ -206,25 +209,23 @@ __global__ void __launch_bounds__(BUILD_THREADS, 1) build_rows_kernel(const Buil
                 const double inv_s = 1.0 / s;
                 for (int t = tid; t < nc; t += BUILD_THREADS) {
                     const int y = t % kprev, a = t / kprev;
-                    stage[env_off(P, 0, a, y)] = sM[t] * inv_s;
+                    stage[env_off(P, 0, a, y)] = sM0[t] * inv_s;
                 }
                 __syncthreads();
                 for (int t = tid; t < TSZ; t += BUILD_THREADS) Aout[t] = stage[t];
                 __syncthreads();
                 break;
             }
-            int nrow = ql;
-            if (nrow & 1) {   // pad to an even row count with a zero row (never happens for c >= 1)
-                for (int t = tid; t < nc; t += BUILD_THREADS) sM[(size_t)nrow * LDM + t] = 0.0;
-                ++nrow;
-                __syncthreads();
-            }
-            double fro2 = 0.0;
+            // M P = Q R with column pivoting (R only); the singular values and right singular vectors of
+            // M are those of R, with the columns permuted back
+            PROF(7);
+            const double fro2 = householder_qrcp<P / 2>(sMc, LDC, ql, nc, sRed, sperm, sS, nullptr);
+            const int nrow = ql < nc ? ql : nc;        // rows of R (even: ql and nc are)
             for (int t = tid; t < nrow * nc; t += BUILD_THREADS) {
-                const double v = sM[(size_t)(t / nc) * LDM + (t % nc)];
-                fro2 += v * v;
+                const int j = t % nc, i = t / nc;
+                sM[(size_t)i * LDM + j] = j >= i ? sMc[i + (size_t)j * LDC] : 0.0;
             }
-            fro2 = block_sum(fro2, sRed);
+            __syncthreads();
             const double thr2 = fro2 * 1e-30;      // sigma <= 1e-15 |M|_F: below the numerical rank
             PROF(4);
             const int nsw = jacobi_rows(sM, LDM, nrow, nc, fro2, thr2, sS, args.flags);
@@ -264,8 +265,9 @@ __global__ void __launch_bounds__(BUILD_THREADS, 1) build_rows_kernel(const Buil
                     // a kept direction below the numerical rank carries no weight (M v = 0 for any
                     // orthonormal completion); it is stored as a zero row
                     const double v = sx * sx > thr2 ? sM[(size_t)x * LDM + col] / sx : 0.0;
-                    sV[(size_t)yp * LDV + col] = v;
-                    stage[env_off(P, yp, col / kprev, col % kprev)] = v;
+                    const int oc = sperm[col];        // original column (a, y) of pivoted column col
+                    sV[(size_t)yp * LDV + oc] = v;
+                    stage[env_off(P, yp, oc / kprev, oc % kprev)] = v;
                 }
             }
             __syncthreads();

@@ -27,13 +27,54 @@ __device__ __forceinline__ double block_sum(double v, double* scratch) {
     return t;
 }
 
-// Given alpha = x_j and ss = sum_{i>j} x_i^2, the Householder reflector H = I - tau v v^T with
-// v_j = 1 that maps x to beta e_j (LAPACK dlarfg convention): returns beta, tau, and the factor
-// that turns x_{i>j} into v_i.
-__device__ __forceinline__ void reflector_scalars(double alpha, double ss, double& beta, double& tau, double& scale) {
+// Quad-cooperative column kernels used by the Householder routines.  A quad (4 lanes, rg = lane & 3)
+// owns one column; lane rg handles rows i0 + rg + 4k.  MAXK = max rows per lane.  Loads are batched
+// into registers (independent accumulators) so that shared-memory latency overlaps.
+template <int MAXK>
+__device__ __forceinline__ double quad_dot_update(const double* __restrict__ v, double* __restrict__ col,
+                                                  int i0, int m, int rg, unsigned qmask, double tau, double head,
+                                                  double& below2) {
+    // w = tau * (head + sum_{i >= i0} v_i col_i);  col_i -= w v_i;  below2 = sum_{i >= i0} col_i^2 (after update)
+    double x[MAXK], vv[MAXK];
+    double w0 = 0.0, w1 = 0.0, w2 = 0.0, w3 = 0.0;
+#pragma unroll
+    for (int k = 0; k < MAXK; ++k) {
+        const int i = i0 + rg + 4 * k;
+        const bool in = i < m;
+        x[k] = in ? col[i] : 0.0;
+        vv[k] = in ? v[i] : 0.0;
+    }
+#pragma unroll
+    for (int k = 0; k < MAXK; k += 4) {
+        w0 = fma(vv[k], x[k], w0);
+        if (k + 1 < MAXK) w1 = fma(vv[k + 1], x[k + 1], w1);
+        if (k + 2 < MAXK) w2 = fma(vv[k + 2], x[k + 2], w2);
+        if (k + 3 < MAXK) w3 = fma(vv[k + 3], x[k + 3], w3);
+    }
+    double w = (w0 + w1) + (w2 + w3);
+    w += __shfl_xor_sync(qmask, w, 1);
+    w += __shfl_xor_sync(qmask, w, 2);
+    w = (w + head) * tau;
+    double s0 = 0.0, s1 = 0.0;
+#pragma unroll
+    for (int k = 0; k < MAXK; ++k) {
+        const int i = i0 + rg + 4 * k;
+        if (i < m) {
+            const double nv = fma(-w, vv[k], x[k]);
+            col[i] = nv;
+            if (k & 1) s1 = fma(nv, nv, s1); else s0 = fma(nv, nv, s0);
+        }
+    }
+    below2 = s0 + s1;
+    return w;
+}
+
+// Reflector from alpha = x_j and nrm2 = sum_{i >= j} x_i^2 (the diagonal entry included, so no
+// cancellation): beta = -sign(alpha) sqrt(nrm2), tau = (beta - alpha) / beta, v_i = x_i / (alpha - beta).
+__device__ __forceinline__ void reflector_from_norm(double alpha, double nrm2, double& beta, double& tau, double& scale) {
     beta = alpha; tau = 0.0; scale = 0.0;
-    if (ss != 0.0) {
-        const double nrm = sqrt(fma(alpha, alpha, ss));
+    if (nrm2 > 0.0) {
+        const double nrm = sqrt(nrm2);
         beta = alpha >= 0.0 ? -nrm : nrm;
         tau = (beta - alpha) / beta;
         scale = 1.0 / (alpha - beta);
@@ -41,11 +82,12 @@ __device__ __forceinline__ void reflector_scalars(double alpha, double ss, doubl
 }
 
 // Householder QR of the m x n column-major matrix X (leading dim ld, odd) in shared memory,
-// n <= 8 * (warps per CTA).  On return the upper trapezoid holds R, the reflector vectors (unit
-// diagonal implied) sit below the diagonal, tau[j] their scalars; kk = min(m,n) reflectors.
-// Step j: every trailing column is updated at once by a quad of lanes (4 interleaved row groups);
-// the quad that owns column j+1 goes on to build reflector j+1 from the freshly updated column,
-// so a step costs one barrier.
+// m <= 4 * MAXK, n <= 8 * (warps per CTA).  On return the upper trapezoid holds R, the reflector
+// vectors (unit diagonal implied) sit below the diagonal, tau[j] their scalars; kk = min(m,n).
+// Step j: every trailing column is updated at once by a quad of lanes; the quad that owns column
+// j+1 goes on to build reflector j+1 from the freshly updated column (its remaining norm comes
+// out of the update for free), so a step costs one barrier.
+template <int MAXK>
 __device__ void householder_qr(double* X, int ld, int m, int n, double* tau) {
     const int kk = m < n ? m : n;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -54,11 +96,11 @@ __device__ void householder_qr(double* X, int ld, int m, int n, double* tau) {
     const int colidx = warp * 8 + cs;
     if (warp == 0) {     // reflector 0
         double ss = 0.0;
-        for (int i = 1 + lane; i < m; i += 32) { const double v = X[i]; ss += v * v; }
+        for (int i = lane; i < m; i += 32) { const double v = X[i]; ss = fma(v, v, ss); }
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
         double bet, t, scale;
-        reflector_scalars(X[0], ss, bet, t, scale);
+        reflector_from_norm(X[0], ss, bet, t, scale);
         __syncwarp();
         for (int i = 1 + lane; i < m; i += 32) X[i] *= scale;
         if (lane == 0) { X[0] = bet; tau[0] = t; }
@@ -70,29 +112,15 @@ __device__ void householder_qr(double* X, int ld, int m, int n, double* tau) {
         const int jj = j + 1 + colidx;
         if (jj < n) {
             double* col = X + (size_t)jj * ld;
-            const bool next = (colidx == 0) && (j + 1 < kk);
-            double nxt = 0.0;
-            if (t != 0.0) {
-                double w = 0.0;
-                for (int i = j + 1 + rg; i < m; i += 4) w = fma(colj[i], col[i], w);
-                w += __shfl_xor_sync(qmask, w, 1);
-                w += __shfl_xor_sync(qmask, w, 2);
-                w = (w + col[j]) * t;
-                for (int i = j + 1 + rg; i < m; i += 4) {
-                    const double v = fma(-w, colj[i], col[i]);
-                    col[i] = v;
-                    if (i > j + 1) nxt = fma(v, v, nxt);
-                }
-                if (rg == 0) col[j] -= w;
-            } else if (next) {
-                for (int i = j + 2 + rg; i < m; i += 4) { const double v = col[i]; nxt = fma(v, v, nxt); }
-            }
-            if (next) {
-                nxt += __shfl_xor_sync(qmask, nxt, 1);
-                nxt += __shfl_xor_sync(qmask, nxt, 2);
-                __syncwarp(qmask);                     // the quad's updates of column j+1 are visible
+            double below2;
+            const double w = quad_dot_update<MAXK>(colj, col, j + 1, m, rg, qmask, t, col[j], below2);
+            if (rg == 0) col[j] -= w;
+            if (colidx == 0 && j + 1 < kk) {       // build reflector j+1 from the updated column
+                below2 += __shfl_xor_sync(qmask, below2, 1);
+                below2 += __shfl_xor_sync(qmask, below2, 2);
+                __syncwarp(qmask);
                 double bet, t1, scale;
-                reflector_scalars(col[j + 1], nxt, bet, t1, scale);
+                reflector_from_norm(col[j + 1], below2, bet, t1, scale);
                 __syncwarp(qmask);
                 for (int i = j + 2 + rg; i < m; i += 4) col[i] *= scale;
                 if (rg == 0) { col[j + 1] = bet; tau[j + 1] = t1; }
@@ -103,6 +131,7 @@ __device__ void householder_qr(double* X, int ld, int m, int n, double* tau) {
 }
 
 // Overwrite the reflectors with the explicit thin Q (m x kk), in place (LAPACK dorg2r order).
+template <int MAXK>
 __device__ void householder_form_q(double* X, int ld, int m, int kk, const double* tau) {
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int cs = lane >> 2, rg = lane & 3;
@@ -114,15 +143,9 @@ __device__ void householder_form_q(double* X, int ld, int m, int kk, const doubl
         const int jj = j + 1 + colidx;
         if (jj < kk) {
             double* col = X + (size_t)jj * ld;
-            double w = 0.0;
-            if (t != 0.0) {
-                // Q[j][jj] is 0 before H_j is applied, so the dot product starts below row j
-                for (int i = j + 1 + rg; i < m; i += 4) w = fma(colj[i], col[i], w);
-                w += __shfl_xor_sync(qmask, w, 1);
-                w += __shfl_xor_sync(qmask, w, 2);
-                w *= t;
-                for (int i = j + 1 + rg; i < m; i += 4) col[i] = fma(-w, colj[i], col[i]);
-            }
+            double below2;
+            // Q[j][jj] is 0 before H_j is applied: head = 0, and the new Q[j][jj] is -w
+            const double w = quad_dot_update<MAXK>(colj, col, j + 1, m, rg, qmask, t, 0.0, below2);
             if (rg == 0) col[j] = -w;
         }
         __syncthreads();
@@ -135,6 +158,79 @@ __device__ void householder_form_q(double* X, int ld, int m, int kk, const doubl
         }
         __syncthreads();
     }
+}
+
+// Householder QR with column pivoting, R only:  X P = Q R  for the m x n column-major X in shared
+// memory (m <= 4 * MAXK, n <= 8 * warps).  On return the upper trapezoid of X holds R (kk = min(m,n)
+// rows), perm[j] the original index of column j.  cn (>= n doubles) is scratch.  Returns
+// sum of squares of X (= |X|_F^2) to all threads.
+// The pivot of step j is the column of largest REMAINING norm; those norms are not downdated but
+// summed afresh inside every trailing update, so they are exact.  Warp 0 picks the pivot, swaps it
+// into place and builds the reflector while the other warps wait: two barriers per step.
+// The point of the pivoting is what it does to the Jacobi SVD that follows ("SVD"):
+// the rows of R are graded and nearly orthogonal, and the sweeps drop from ~12 to ~5.
+template <int MAXK>
+__device__ double householder_qrcp(double* X, int ld, int m, int n, double* cn, int* perm, double* tau, int* ipiv) {
+    const int kk = m < n ? m : n;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int cs = lane >> 2, rg = lane & 3;
+    const unsigned qmask = 0xfu << (lane & ~3);
+    const int colidx = warp * 8 + cs;
+    if (colidx < n) {
+        const double* col = X + (size_t)colidx * ld;
+        double s0 = 0.0, s1 = 0.0;
+        for (int i = rg; i < m; i += 8) {
+            const double a = col[i]; s0 = fma(a, a, s0);
+            if (i + 4 < m) { const double b = col[i + 4]; s1 = fma(b, b, s1); }
+        }
+        double ss = s0 + s1;
+        ss += __shfl_xor_sync(qmask, ss, 1);
+        ss += __shfl_xor_sync(qmask, ss, 2);
+        if (rg == 0) { cn[colidx] = ss; perm[colidx] = colidx; }
+    }
+    __syncthreads();
+    double fro2 = 0.0;
+    for (int jj = 0; jj < n; ++jj) fro2 += cn[jj];
+    for (int j = 0; j < kk; ++j) {
+        if (warp == 0) {
+            // pivot: argmax of the remaining norms over columns j..n-1 (smallest index on ties)
+            double best = -1.0; int bi = j;
+            for (int jj = j + lane; jj < n; jj += 32) { const double v = cn[jj]; if (v > best) { best = v; bi = jj; } }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                const double ov = __shfl_xor_sync(0xffffffffu, best, o);
+                const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+                if (ov > best || (ov == best && oi < bi)) { best = ov; bi = oi; }
+            }
+            double* cj = X + (size_t)j * ld;
+            double* cp = X + (size_t)bi * ld;
+            if (bi != j) {
+                for (int i = lane; i < m; i += 32) { const double a = cj[i]; cj[i] = cp[i]; cp[i] = a; }
+                if (lane == 0) { cn[bi] = cn[j]; const int t = perm[j]; perm[j] = perm[bi]; perm[bi] = t; }
+            }
+            __syncwarp();
+            double bet, t, scale;
+            reflector_from_norm(cj[j], best, bet, t, scale);
+            __syncwarp();
+            for (int i = j + 1 + lane; i < m; i += 32) cj[i] *= scale;
+            if (lane == 0) { cj[j] = bet; tau[j] = t; }
+        }
+        __syncthreads();
+        const double* colj = X + (size_t)j * ld;
+        const double t = tau[j];
+        const int jj = j + 1 + colidx;
+        if (jj < n) {
+            double* col = X + (size_t)jj * ld;
+            double below2;
+            const double w = quad_dot_update<MAXK>(colj, col, j + 1, m, rg, qmask, t, col[j], below2);
+            below2 += __shfl_xor_sync(qmask, below2, 1);
+            below2 += __shfl_xor_sync(qmask, below2, 2);
+            if (rg == 0) { col[j] -= w; cn[jj] = below2; }
+        }
+        __syncthreads();
+    }
+    (void)ipiv;
+    return fro2;
 }
 
 // One-sided (Hestenes) Jacobi on the ROWS of the n x nc row-major matrix M (row length ld, a
@@ -217,16 +313,19 @@ __device__ int jacobi_rows(double* M, int ld, int n, int nc, double fro2, double
                 double* x = M + (size_t)r1 * ld;
                 double* y = M + (size_t)r2 * ld;
                 double2 xv[4], yv[4];
-                double g = 0.0;
+                double gp[4] = {0.0, 0.0, 0.0, 0.0};
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
                     const int c = c0 + 16 * k;
                     if (c < nc) {
                         xv[k] = *reinterpret_cast<const double2*>(x + c);
                         yv[k] = *reinterpret_cast<const double2*>(y + c);
-                        g = fma(xv[k].x, yv[k].x, g); g = fma(xv[k].y, yv[k].y, g);
                     }
                 }
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                    if (c0 + 16 * k < nc) gp[k] = fma(xv[k].y, yv[k].y, xv[k].x * yv[k].x);
+                double g = (gp[0] + gp[1]) + (gp[2] + gp[3]);
 #pragma unroll
                 for (int o = 4; o > 0; o >>= 1) g += __shfl_xor_sync(gmask, g, o);
                 const double mx = a > b ? a : b, ab = a * b, g2 = g * g;
@@ -252,39 +351,37 @@ __device__ int jacobi_rows(double* M, int ld, int n, int nc, double fro2, double
 #ifdef TNMC_PROFILE
                     jacc[9] += 1;
 #endif
-                    double sx2 = 0.0, sy2 = 0.0;
 #pragma unroll
                     for (int k = 0; k < 4; ++k) {
                         const int c = c0 + 16 * k;
                         if (c < nc) {
                             double2 xn, yn;
-                            xn.x = cs * xv[k].x - sn * yv[k].x;  yn.x = sn * xv[k].x + cs * yv[k].x;
-                            xn.y = cs * xv[k].y - sn * yv[k].y;  yn.y = sn * xv[k].y + cs * yv[k].y;
+                            xn.x = fma(cs, xv[k].x, -sn * yv[k].x);  yn.x = fma(sn, xv[k].x, cs * yv[k].x);
+                            xn.y = fma(cs, xv[k].y, -sn * yv[k].y);  yn.y = fma(sn, xv[k].y, cs * yv[k].y);
                             xv[k] = xn; yv[k] = yn;
-                            sx2 = fma(xn.x, xn.x, sx2); sx2 = fma(xn.y, xn.y, sx2);
-                            sy2 = fma(yn.x, yn.x, sy2); sy2 = fma(yn.y, yn.y, sy2);
+                            *reinterpret_cast<double2*>(x + c) = xn;
+                            *reinterpret_cast<double2*>(y + c) = yn;
                         }
                     }
                     // new squared norms by the 2x2 congruence; where one of them came out of a
-                    // cancellation (a row was nearly annihilated) take the directly summed value
+                    // cancellation (a row was nearly annihilated) sum it directly
                     const double cc = cs * cs, ss = sn * sn, csg = 2.0 * cs * sn * g;
                     double na = cc * a - csg + ss * b;
                     double nb = ss * a + csg + cc * b;
                     if (na < 1e-4 * mx || nb < 1e-4 * mx) {
+                        double sx2 = 0.0, sy2 = 0.0;
+#pragma unroll
+                        for (int k = 0; k < 4; ++k)
+                            if (c0 + 16 * k < nc) {
+                                sx2 = fma(xv[k].x, xv[k].x, sx2); sx2 = fma(xv[k].y, xv[k].y, sx2);
+                                sy2 = fma(yv[k].x, yv[k].x, sy2); sy2 = fma(yv[k].y, yv[k].y, sy2);
+                            }
 #pragma unroll
                         for (int o = 4; o > 0; o >>= 1) {
                             sx2 += __shfl_xor_sync(gmask, sx2, o);
                             sy2 += __shfl_xor_sync(gmask, sy2, o);
                         }
                         na = sx2; nb = sy2;
-                    }
-#pragma unroll
-                    for (int k = 0; k < 4; ++k) {
-                        const int c = c0 + 16 * k;
-                        if (c < nc) {
-                            *reinterpret_cast<double2*>(x + c) = xv[k];
-                            *reinterpret_cast<double2*>(y + c) = yv[k];
-                        }
                     }
                     if (t8 == 0) { nrm2[r1] = na; nrm2[r2] = nb; }
                     JPROF(12);
