@@ -98,7 +98,7 @@ static cudaError_t launch_build_t(const tnmc_ctx* ctx, const BuildArgs& a, int d
     const size_t smem = BuildCfg<P>::smem_bytes(a.L);
     cudaError_t e = cudaFuncSetAttribute(build_rows_kernel<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    build_rows_kernel<P><<<dis_count, BUILD_THREADS, smem, ctx->stream>>>(a);
+    build_rows_kernel<P><<<dis_count, BuildCfg<P>::NT, smem, ctx->stream>>>(a);
     return cudaPeekAtLastError();
 }
 

@@ -1,20 +1,26 @@
 // tnmc_build.cuh -- boundary-MPS environment build (steps a-1..a-7 of DESIGN.md).
 //
 // One CTA per disorder realisation walks the rows bottom -> top and, per row,
-//   1. applies the row MPO (Eq. 7-8) site by site, fused with
-//   2. the left->right canonicalising Householder QR sweep (P-C2 step 1), then
-//   3. the right->left truncated SVD sweep (P-C2 step 2; one-sided Jacobi on the rows of the
-//      D_l x 2D_r matrix) and the final scale (P-C2 step 3).
-// The MPO tensors are never materialised: with W[l,a,r,d] = delta(l,a) B_r[a,r] B_d[a,d]
-// the product tensor is  A'[(l,i),a,(r,k)] = delta(l,a) B_r[a,r] C_a[i,k],
-// C_a = sum_m B_d[a,m] A[i,m,k], so the carried R of the QR sweep only ever meets C_a.
+//   A. applies the row MPO (Eq. 7-8) site by site, fused with the left->right
+//      canonicalising QR sweep (P-C2 step 1), then
+//   B. runs the right->left truncated SVD sweep (P-C2 step 2) and the final scale (P-C2 step 3).
+// The MPO tensors are never materialised.  With W[l,a,r,d] = delta(l,a) B_r[a,r] B_d[a,d] the
+// product tensor is  A'[(l,i),a,(r,k)] = delta(l,a) B_r[a,r] C_a[i,k],  C_a = sum_m B_d[a,m] A[i,m,k],
+// so with the carried factor R = [R_0 | R_1] (column blocks l = 0, 1) the QR operand of a site is
+//   X[(x,a),(r,k)] = B_r[a,r] T_a[x,k],  T_a = R_a C_a,   i.e.  X = blockdiag(T_0, T_1) (B_r (x) 1).
+// B_r (x) 1 is invertible, so an orthonormal basis of X's columns is blockdiag(Q_0, Q_1) with
+// T_a = Q_a R'_a: TWO independent thin QRs of half the size (4x fewer flops, half the depth), run
+// side by side by the two halves of the CTA.  The factor pushed right is
+// R_new[(a,y),(r,k)] = B_r[a,r] R'_a[y,k] (not triangular -- it need not be: any orthonormal basis
+// of the left block is an equally good gauge for the SVD sweep).
+// Q_a is never formed: the SVD sweep applies its reflectors to [Pc_a; 0] directly,
+//   M = [Q_0 Pc_0 | Q_1 Pc_1]   (Pc = M V_k carried from the site to the right),
+// column by column with no barrier between reflectors.
 #pragma once
 #include "tnmc_common.cuh"
 #include "tnmc_linalg.cuh"
 
 namespace tnmc {
-
-constexpr int BUILD_THREADS = 256;
 
 #ifdef TNMC_PROFILE
 #define PROF_DECL long long prof_t0 = clock64();
@@ -35,47 +41,54 @@ struct BuildArgs {
     const int* slot_of_row;      // [L] device: env slot of each row for this pass (-1: not stored)
     double* env;                 // env base
     size_t env_dis_stride;       // doubles per disorder (n_slots * L * 2P^2)
-    double* qbuf;                // scratch, per disorder L * (LDX * D) doubles
+    double* qbuf;                // scratch, per disorder L * QSZ doubles (reflectors of the QR sweep)
     double* logscale;            // (n_dis, L): logscale of every row (written for rows built)
     unsigned long long* flags;
 };
 
 template <int P>
 struct BuildCfg {
+    static constexpr int NT = 8 * P;          // threads per CTA: one quad per column of a 2P-column matrix
     static constexpr int D = 2 * P;           // doubled bond
-    static constexpr int LDX = 2 * D + 1;     // leading dim of the column-major QR operand (odd: no bank conflicts)
-    static constexpr int LDM = 2 * P;         // row length of the Jacobi operand (row-major)
-    static constexpr int LDV = 2 * P + 1;     // padded row length of the selected right singular vectors
+    static constexpr int LDX = D + 4;         // column-major leading dim (= 4 mod 16: a half-warp of 4 quads hits 16 distinct 8-byte banks)
+    static constexpr int LDM = D + 2;         // row length of the Jacobi operand (row-major)
+    static constexpr int LDV = D + 1;         // row length of the selected right singular vectors
+    static constexpr int LDR = P + 1;         // row length of the carried R_a[x][i]
+    static constexpr int LDU = P + 1;         // row length of the carried Pc[z][y]
     static constexpr int TSZ = 2 * P * P;     // doubles per stored site tensor
-    static constexpr int QSZ = LDX * D;       // doubles per site of the Q scratch
+    static constexpr int QSZ = LDX * D + D;   // doubles per site of the reflector scratch: image of X + tau
     // shared-memory carve-up (doubles)
-    static constexpr int X_OFF = 0;                   // LDX*D : QR operand / Q_c / staging
-    static constexpr int R_OFF = X_OFF + LDX * D;     // D*LDC : carried R [x][lambda] (ld D) / column-major M for QRCP (ld LDC)
-    static constexpr int LDC = D + 1;         // leading dim of the column-major copy of M that QRCP works on
-    static constexpr int A_OFF = R_OFF + D * LDC;     // TSZ   : lower-row site tensor (fragment order) / Pc
-    static constexpr int C_OFF = A_OFF + TSZ;         // TSZ   : C_a[i][k] / Pc_new
-    static constexpr int M0_OFF = C_OFF + TSZ;        // D*LDM : copy of M before rotation
-    static constexpr int S_OFF = M0_OFF + D * LDM;    // 2*D + 8 : tau / sigma / scalars
-    static constexpr int N_DBL = S_OFF + 2 * D + 8;
+    static constexpr int X_OFF = 0;                       // LDX*D : T_0 | T_1 (QR sweep); M, then stage + V_k (SVD sweep)
+    static constexpr int Y_OFF = X_OFF + LDX * D;         // D*LDM >= 2*D*LDR, LDX*D : carried R (QR sweep); reflectors, then Jacobi operand
+    static constexpr int Y_SZ = (D * LDM > LDX * D ? D * LDM : LDX * D);
+    static constexpr int Z_OFF = Y_OFF + Y_SZ;            // D*D   : site tensor staging (QR sweep); M before rotation (SVD sweep)
+    static constexpr int U_OFF = Z_OFF + D * D;           // D*LDU : C_a (QR sweep); carried Pc / M V_k (SVD sweep)
+    static constexpr int S_OFF = U_OFF + D * LDU;         // 3*D + 40 : tau / column norms / sigma / reduction scratch
+    static constexpr int N_DBL = S_OFF + 3 * D + 40;
     static size_t smem_bytes(int L) { return sizeof(double) * N_DBL + sizeof(int) * (L + 2 + 2 * D); }
 };
 
 template <int P>
-__global__ void __launch_bounds__(BUILD_THREADS, 1) build_rows_kernel(const BuildArgs args) {
+__global__ void __launch_bounds__(BuildCfg<P>::NT, 1) build_rows_kernel(const BuildArgs args) {
     using Cfg = BuildCfg<P>;
-    constexpr int D = Cfg::D, LDX = Cfg::LDX, LDM = Cfg::LDM, LDV = Cfg::LDV, TSZ = Cfg::TSZ, LDC = Cfg::LDC;
+    constexpr int NT = Cfg::NT, HALF = NT / 2, D = Cfg::D, LDX = Cfg::LDX, LDM = Cfg::LDM, LDV = Cfg::LDV,
+                  LDR = Cfg::LDR, LDU = Cfg::LDU, TSZ = Cfg::TSZ;
+    constexpr int MAXK = P / 2;          // rows per quad lane: every matrix here has at most D = 4 MAXK rows
     extern __shared__ __align__(16) double smem[];
     double* sX = smem + Cfg::X_OFF;
-    double* sR = smem + Cfg::R_OFF;
-    double* sA = smem + Cfg::A_OFF;
-    double* sC = smem + Cfg::C_OFF;
-    double* sM0 = smem + Cfg::M0_OFF;
-    double* sS = smem + Cfg::S_OFF;      // [0,D): tau / sigma   [D, 2D): reduction scratch
-    double* sRed = sS + D;
-    int* sq = reinterpret_cast<int*>(smem + Cfg::N_DBL);   // [L+1] QR bond dims
-    int* spos = sq + args.L + 2;                           // [2D] rank / position of each Jacobi row
+    double* sY = smem + Cfg::Y_OFF;
+    double* sZ = smem + Cfg::Z_OFF;
+    double* sU = smem + Cfg::U_OFF;
+    double* sTau = smem + Cfg::S_OFF;    // [D]  tau of block a at a*P (QR sweep) / of the QRCP
+    double* sCn = sTau + D;              // [D]  remaining column norms of the QRCP
+    double* sSig = sCn + D;              // [D]  squared row norms of the Jacobi, then sigma
+    double* sRed = sSig + D;             // [40] block reduction scratch
+    int* sq = reinterpret_cast<int*>(smem + Cfg::N_DBL);   // [L+1] rows q_c of the carried R = left bond of Q_c
+    int* spos = sq + args.L + 2;                           // [D] rank / position of each Jacobi row
+    int* sperm = spos + D;                                 // [D] column permutation of the QRCP
 
     const int tid = threadIdx.x;
+    const int half = tid >= HALF ? 1 : 0, gt = tid - half * HALF;
     const int d = args.dis_begin + blockIdx.x;
     const int L = args.L, chi = args.chi;
     const double beta = args.beta;
@@ -89,167 +102,186 @@ __global__ void __launch_bounds__(BUILD_THREADS, 1) build_rows_kernel(const Buil
         double* env_out = env_d + (size_t)args.slot_of_row[r] * L * TSZ;
         double logs = 0.0;   // all threads carry the same value
 
-        // ------------------------------------------------------------------ QR sweep, left -> right
-        if (tid == 0) { sq[0] = 1; sR[0] = 1.0; sR[1] = 1.0; }
+        // ------------------------------------------------------------------ A. QR sweep, left -> right
+        double* sR = sY;     // carried R_a[x][i] at a*D*LDR, row length LDR
+        if (tid == 0) { sq[0] = 1; sR[0] = 1.0; sR[D * LDR] = 1.0; }
         __syncthreads();
         for (int c = 0; c < L; ++c) {
             const int bl = row_bond(L, chi, r + 1, c), br = row_bond(L, chi, r + 1, c + 1);
-            const int ql = sq[c], m = 2 * ql;
-            const int nr = (c == L - 1) ? 1 : 2, n = nr * br;
+            const int q = sq[c];
             const double* Ain = env_in + (size_t)c * TSZ;
-            for (int t = tid; t < TSZ; t += BUILD_THREADS) sA[t] = Ain[t];
+            for (int t = tid; t < TSZ; t += NT) sZ[t] = Ain[t];
             __syncthreads();
             {   // C_a[i][k] = sum_m B_d[a][m] A[i][m][k]      (Eq. 7: B_d[a][m] = exp(beta Jd (2a-1)(2m-1)))
                 const int jd = args.J.jd(d, r, c);
                 const double w_same = exp(beta * jd), w_diff = exp(-beta * jd);
-                for (int t = tid; t < 2 * bl * br; t += BUILD_THREADS) {
+                for (int t = tid; t < 2 * bl * br; t += NT) {
                     const int k = t % br, i = (t / br) % bl, a = t / (br * bl);
-                    sC[(a * P + i) * P + k] = w_same * sA[env_off(P, i, a, k)] + w_diff * sA[env_off(P, i, 1 - a, k)];
+                    sU[(a * P + i) * LDU + k] = w_same * sZ[env_off(P, i, a, k)] + w_diff * sZ[env_off(P, i, 1 - a, k)];
                 }
             }
             __syncthreads();
-            {   // X[(2x+a), (rr*br+k)] = B_r[a][rr] * sum_i R[x][a*bl+i] C_a[i][k]
-                const int jr = (c == L - 1) ? 0 : args.J.jr(d, r, c);
-                const double w_same = exp(beta * jr), w_diff = exp(-beta * jr);
-                for (int t = tid; t < m * br; t += BUILD_THREADS) {
-                    const int k = t % br, a = (t / br) & 1, x = t / (2 * br);
-                    const double* Rrow = sR + (size_t)x * D + a * bl;
-                    const double* Ccol = sC + (size_t)a * P * P + k;
-                    double acc = 0.0;
-                    for (int i = 0; i < bl; ++i) acc += Rrow[i] * Ccol[i * P];
-                    const int row = 2 * x + a;
-                    if (nr == 1) sX[row + (size_t)k * LDX] = acc;
-                    else {
-                        sX[row + (size_t)((a)*br + k) * LDX] = w_same * acc;       // rr == a
-                        sX[row + (size_t)((1 - a) * br + k) * LDX] = w_diff * acc; // rr != a
-                    }
+            // T_a[x][k] = sum_i R_a[x][i] C_a[i][k]  -> column k of block a of X
+            for (int t = tid; t < 2 * q * br; t += NT) {
+                const int x = t % q, k = (t / q) % br, a = t / (q * br);
+                const double* Rrow = sR + (size_t)a * D * LDR + (size_t)x * LDR;
+                const double* Ccol = sU + (size_t)a * P * LDU + k;
+                double acc0 = 0.0, acc1 = 0.0;
+                int i = 0;
+                for (; i + 1 < bl; i += 2) {
+                    acc0 = fma(Rrow[i], Ccol[i * LDU], acc0);
+                    acc1 = fma(Rrow[i + 1], Ccol[(i + 1) * LDU], acc1);
                 }
+                if (i < bl) acc0 = fma(Rrow[i], Ccol[i * LDU], acc0);
+                sX[(size_t)(a * P + k) * LDX + x] = acc0 + acc1;
             }
             __syncthreads();
             double* Qout = qbuf_d + (size_t)c * Cfg::QSZ;
             if (c == L - 1) {
-                // last site: not orthogonalised (P-C2 step 1 stops at L-2); it now carries the norm
-                for (int t = tid; t < m; t += BUILD_THREADS) Qout[t] = sX[t];
+                // last site (br = 1): not orthogonalised (P-C2 step 1 stops at L-2); T_a[:,0] is column a of its M
+                for (int t = tid; t < 2 * q; t += NT) {
+                    const int x = t % q, a = t / q;
+                    Qout[(size_t)(a * P) * LDX + x] = sX[(size_t)(a * P) * LDX + x];
+                }
                 if (tid == 0) sq[L] = 1;
                 __syncthreads();
                 break;
             }
             PROF(0);
-            householder_qr<P>(sX, LDX, m, n, sS);
+            const int p = q < br ? q : br;
+            householder_qr_g<MAXK>(sX + (size_t)half * P * LDX, LDX, q, br, sTau + half * P, gt, HALF, 1 + half);
+            __syncthreads();
             PROF(1);
-            const int kk = m < n ? m : n;
-            // R -> carried R/|R|_F for the next site; logscale += log |R|_F
+            // R_new[(a,y)][(rr,k)] = B_r[a][rr] R'_a[y][k] / |R_new|_F;  logscale += log |R_new|_F
+            const int jr = args.J.jr(d, r, c);
+            const double w_same = exp(beta * jr), w_diff = exp(-beta * jr);
             double ss = 0.0;
-            for (int t = tid; t < kk * n; t += BUILD_THREADS) {
-                const int x = t / n, lam = t % n;
-                const double v = lam >= x ? sX[x + (size_t)lam * LDX] : 0.0;
-                ss += v * v;
+            for (int t = tid; t < 2 * p * br; t += NT) {
+                const int y = t % p, k = (t / p) % br, a = t / (p * br);
+                const double v = k >= y ? sX[(size_t)(a * P + k) * LDX + y] : 0.0;
+                ss = fma(v, v, ss);
             }
-            ss = block_sum(ss, sRed);
+            ss = block_sum(ss, sRed) * (w_same * w_same + w_diff * w_diff);
             const double s = sqrt(ss);
             if (!(s > 0.0) || !isfinite(s)) { if (tid == 0) raise_flag(args.flags, FLAG_NONFINITE); }
             logs += log(s);
             const double inv_s = 1.0 / s;
-            for (int t = tid; t < kk * n; t += BUILD_THREADS) {
-                const int x = t / n, lam = t % n;
-                sR[(size_t)x * D + lam] = lam >= x ? sX[x + (size_t)lam * LDX] * inv_s : 0.0;
+            for (int t = tid; t < 2 * p * br; t += NT) {
+                const int k = t % br, y = (t / br) % p, a = t / (p * br);
+                const double v = k >= y ? sX[(size_t)(a * P + k) * LDX + y] * inv_s : 0.0;
+                sR[(size_t)a * D * LDR + (size_t)(a * p + y) * LDR + k] = w_same * v;          // rr == a
+                sR[(size_t)(1 - a) * D * LDR + (size_t)(a * p + y) * LDR + k] = w_diff * v;    // rr != a
             }
-            if (tid == 0) sq[c + 1] = kk;
+            if (tid == 0) sq[c + 1] = 2 * p;
+            // reflectors (below the diagonal of each block) and tau -> scratch for the SVD sweep
+            for (int t = tid; t < 2 * q * p; t += NT) {
+                const int x = t % q, z = (t / q) % p, a = t / (q * p);
+                Qout[(size_t)(a * P + z) * LDX + x] = sX[(size_t)(a * P + z) * LDX + x];
+            }
+            for (int t = tid; t < 2 * p; t += NT) {
+                const int z = t % p, a = t / p;
+                Qout[LDX * D + a * P + z] = sTau[a * P + z];
+            }
             __syncthreads();
             PROF(2);
-            householder_form_q<P>(sX, LDX, m, kk, sS);
-            PROF(3);
-            for (int t = tid; t < m * kk; t += BUILD_THREADS) {
-                const int row = t % m, col = t / m;
-                Qout[row + (size_t)col * LDX] = sX[row + (size_t)col * LDX];
-            }
-            __syncthreads();
         }
 
-        // ------------------------------------------------------------------ SVD sweep, right -> left
-        double* sMc = sR;         // M, column-major [x + col*LDC]: QRCP operand
-        double* sM = sX;          // Jacobi operand (rows of R), row-major, ld = LDM; lives in sX once Q_c is consumed
-        int* sperm = spos + D;    // column permutation of the QRCP
-        double* sPc = sA;         // carried M V_k of the site to the right: [z][y], ld = P
-        double* sPn = sC;
+        // ------------------------------------------------------------------ B. SVD sweep, right -> left
+        double* sMj = sY;             // Jacobi operand (rows of R), row-major, row length LDM
+        double* sM0 = sZ;             // M before rotation, column-major, leading dim D
+        double* stage = sX;           // output tensor in fragment order (once the QRCP result has left X)
+        double* sV = sX + TSZ;        // [y'][col], row length LDV: selected right singular vectors
         int kprev = 1;
-        if (tid == 0) sPc[0] = 1.0;
-        __syncthreads();
         for (int c = L - 1; c >= 0; --c) {
-            const int ql = sq[c], m = 2 * ql, qr = sq[c + 1];
-            const double* Qin = qbuf_d + (size_t)c * Cfg::QSZ;
-            for (int t = tid; t < m * qr; t += BUILD_THREADS) {
-                const int row = t % m, col = t / m;
-                sX[row + (size_t)col * LDX] = Qin[row + (size_t)col * LDX];
-            }
-            __syncthreads();
+            const int q = sq[c];
             const int nc = 2 * kprev;
-            // M[x][a*kprev+y] = sum_z Q_c[(2x+a)][z] Pc[z][y]
-            for (int t = tid; t < ql * nc; t += BUILD_THREADS) {
-                const int y = t % kprev, a = (t / kprev) & 1, x = t / nc;
-                const double* Xrow = sX + (2 * x + a);
-                double acc = 0.0;
-                for (int z = 0; z < qr; ++z) acc += Xrow[(size_t)z * LDX] * sPc[z * P + y];
-                sMc[x + (size_t)(a * kprev + y) * LDC] = acc;
-                sM0[(size_t)x * LDM + a * kprev + y] = acc;
+            const double* Qin = qbuf_d + (size_t)c * Cfg::QSZ;
+            if (c == L - 1) {
+                for (int t = tid; t < 2 * q; t += NT) {
+                    const int x = t % q, a = t / q;
+                    sX[(size_t)a * LDX + x] = Qin[(size_t)(a * P) * LDX + x];
+                }
+            } else {
+                // M = [Q_0 Pc_0 | Q_1 Pc_1]: reflectors of block a applied to [Pc_a; 0]
+                const int p = sq[c + 1] >> 1;
+                for (int t = tid; t < 2 * q * p; t += NT) {
+                    const int x = t % q, z = (t / q) % p, a = t / (q * p);
+                    sY[(size_t)(a * P + z) * LDX + x] = Qin[(size_t)(a * P + z) * LDX + x];
+                }
+                for (int t = tid; t < 2 * p; t += NT) {
+                    const int z = t % p, a = t / p;
+                    sTau[a * P + z] = Qin[LDX * D + a * P + z];
+                }
+                for (int t = tid; t < q * nc; t += NT) {
+                    const int x = t % q, col = t / q;
+                    const int a = col / kprev, y = col - a * kprev;
+                    sX[(size_t)col * LDX + x] = x < p ? sU[(size_t)(a * p + x) * LDU + y] : 0.0;
+                }
+                __syncthreads();
+                householder_apply_g<MAXK>(sY + (size_t)half * P * LDX, LDX, sTau + half * P, q, p,
+                                          sX + (size_t)half * kprev * LDX, LDX, kprev, gt, HALF, 1 + half);
             }
             __syncthreads();
-            double* stage = sX + D * LDM;       // TSZ doubles: output tensor in fragment order
-            double* sV = stage + TSZ;           // [y'][col], ld = LDV: selected right singular vectors
-            for (int t = tid; t < TSZ; t += BUILD_THREADS) stage[t] = 0.0;
             double* Aout = env_out + (size_t)c * TSZ;
             if (c == 0) {
-                // P-C2 step 3: A_0 (1,2,k_1) = Q_0 Pc; divide by its norm, add log to logscale
+                // P-C2 step 3: A_0 (1,2,k_1) = M (1 x nc); divide by its norm, add log to logscale
                 double ss = 0.0;
-                for (int t = tid; t < nc; t += BUILD_THREADS) ss += sM0[t] * sM0[t];
+                for (int t = tid; t < nc; t += NT) { const double v = sX[(size_t)t * LDX]; ss = fma(v, v, ss); }
                 ss = block_sum(ss, sRed);
                 const double s = sqrt(ss);
                 if (!(s > 0.0) || !isfinite(s)) { if (tid == 0) raise_flag(args.flags, FLAG_NONFINITE); }
                 logs += log(s);
                 const double inv_s = 1.0 / s;
-                for (int t = tid; t < nc; t += BUILD_THREADS) {
-                    const int y = t % kprev, a = t / kprev;
-                    stage[env_off(P, 0, a, y)] = sM0[t] * inv_s;
-                }
+                const double m0 = tid < nc ? sX[(size_t)tid * LDX] * inv_s : 0.0;
                 __syncthreads();
-                for (int t = tid; t < TSZ; t += BUILD_THREADS) Aout[t] = stage[t];
+                for (int t = tid; t < TSZ; t += NT) stage[t] = 0.0;
+                __syncthreads();
+                if (tid < nc) stage[env_off(P, 0, tid / kprev, tid % kprev)] = m0;
+                __syncthreads();
+                for (int t = tid; t < TSZ; t += NT) Aout[t] = stage[t];
                 __syncthreads();
                 break;
             }
+            for (int t = tid; t < q * nc; t += NT) {
+                const int x = t % q, col = t / q;
+                sM0[(size_t)col * D + x] = sX[(size_t)col * LDX + x];
+            }
+            PROF(7);
             // M P = Q R with column pivoting (R only); the singular values and right singular vectors of
             // M are those of R, with the columns permuted back
-            PROF(7);
-            const double fro2 = householder_qrcp<P / 2>(sMc, LDC, ql, nc, sRed, sperm, sS, nullptr);
-            const int nrow = ql < nc ? ql : nc;        // rows of R (even: ql and nc are)
-            for (int t = tid; t < nrow * nc; t += BUILD_THREADS) {
+            const double fro2 = householder_qrcp<MAXK>(sX, LDX, q, nc, sCn, sperm, sTau, nullptr);
+            const int nrow = q < nc ? q : nc;        // rows of R (even: q and nc are)
+            for (int t = tid; t < nrow * nc; t += NT) {
                 const int j = t % nc, i = t / nc;
-                sM[(size_t)i * LDM + j] = j >= i ? sMc[i + (size_t)j * LDC] : 0.0;
+                sMj[(size_t)i * LDM + j] = j >= i ? sX[i + (size_t)j * LDX] : 0.0;
             }
             __syncthreads();
             const double thr2 = fro2 * 1e-30;      // sigma <= 1e-15 |M|_F: below the numerical rank
             PROF(4);
-            const int nsw = jacobi_rows(sM, LDM, nrow, nc, fro2, thr2, sS, args.flags);
+            const int nsw = jacobi_rows(sMj, LDM, nrow, nc, fro2, thr2, sSig, args.flags);
             PROF(5);
             PROF_ADD(8, nsw); PROF_ADD(9, 1);
+            (void)nsw;
             // singular values = row norms
             {
                 const int grp = tid >> 3, t8 = tid & 7;
-                for (int x = grp; x < nrow; x += (BUILD_THREADS >> 3)) {
+                for (int x = grp; x < nrow; x += (NT >> 3)) {
                     double a = 0.0;
-                    for (int cc = t8; cc < nc; cc += 8) { const double v = sM[(size_t)x * LDM + cc]; a += v * v; }
+                    for (int cc = t8; cc < nc; cc += 8) { const double v = sMj[(size_t)x * LDM + cc]; a = fma(v, v, a); }
 #pragma unroll
                     for (int o = 4; o > 0; o >>= 1) a += __shfl_xor_sync(0xffu << ((tid & 31) & ~7), a, o);
-                    if (t8 == 0) sS[x] = sqrt(a);
+                    if (t8 == 0) sSig[x] = sqrt(a);
                 }
             }
+            for (int t = tid; t < TSZ; t += NT) stage[t] = 0.0;
             __syncthreads();
-            int k = chi < ql ? chi : ql;
+            int k = chi < q ? chi : q;
             if (nc < k) k = nc;
-            for (int x = tid; x < nrow; x += BUILD_THREADS) {
-                const double sx = sS[x];
+            for (int x = tid; x < nrow; x += NT) {
+                const double sx = sSig[x];
                 int rank = 0;
                 for (int y = 0; y < nrow; ++y) {
-                    const double sy = sS[y];
+                    const double sy = sSig[y];
                     rank += (sy > sx) || (sy == sx && y < x);
                 }
                 spos[x] = rank < k ? rank : -1;
@@ -257,32 +289,34 @@ __global__ void __launch_bounds__(BUILD_THREADS, 1) build_rows_kernel(const Buil
             }
             __syncthreads();
             // A_c[y'][a][y] = v_{y'}  (rows of V_k^T), staged in fragment order and as plain rows
-            for (int t = tid; t < nrow * nc; t += BUILD_THREADS) {
+            for (int t = tid; t < nrow * nc; t += NT) {
                 const int col = t % nc, x = t / nc;
                 const int yp = spos[x];
                 if (yp >= 0) {
-                    const double sx = sS[x];
+                    const double sx = sSig[x];
                     // a kept direction below the numerical rank carries no weight (M v = 0 for any
                     // orthonormal completion); it is stored as a zero row
-                    const double v = sx * sx > thr2 ? sM[(size_t)x * LDM + col] / sx : 0.0;
+                    const double v = sx * sx > thr2 ? sMj[(size_t)x * LDM + col] / sx : 0.0;
                     const int oc = sperm[col];        // original column (a, y) of pivoted column col
                     sV[(size_t)yp * LDV + oc] = v;
                     stage[env_off(P, yp, oc / kprev, oc % kprev)] = v;
                 }
             }
             __syncthreads();
-            for (int t = tid; t < TSZ; t += BUILD_THREADS) Aout[t] = stage[t];
-            // Pn[x][y'] = sum_col M0[x][col] V_k[col][y']   (= M V_k, projector form of P-C2 step 2)
-            for (int t = tid; t < ql * k; t += BUILD_THREADS) {
-                const int yp = t % k, x = t / k;
-                const double* mrow = sM0 + (size_t)x * LDM;
+            for (int t = tid; t < TSZ; t += NT) Aout[t] = stage[t];
+            // Pc_next[x][y'] = sum_col M[x][col] V_k[col][y']   (= M V_k, projector form of P-C2 step 2)
+            for (int t = tid; t < q * k; t += NT) {
+                const int x = t % q, yp = t / q;
+                const double* mcol = sM0 + x;
                 const double* vrow = sV + (size_t)yp * LDV;
-                double acc = 0.0;
-                for (int col = 0; col < nc; ++col) acc += mrow[col] * vrow[col];
-                sPn[x * P + yp] = acc;
+                double acc0 = 0.0, acc1 = 0.0;
+                for (int col = 0; col < nc; col += 2) {
+                    acc0 = fma(mcol[(size_t)col * D], vrow[col], acc0);
+                    acc1 = fma(mcol[(size_t)(col + 1) * D], vrow[col + 1], acc1);
+                }
+                sU[(size_t)x * LDU + yp] = acc0 + acc1;
             }
             __syncthreads();
-            { double* t = sPc; sPc = sPn; sPn = t; }
             kprev = k;
             PROF(6);
         }

@@ -74,9 +74,12 @@ __device__ __forceinline__ double quad_dot_update(const double* __restrict__ v, 
 __device__ __forceinline__ void reflector_from_norm(double alpha, double nrm2, double& beta, double& tau, double& scale) {
     beta = alpha; tau = 0.0; scale = 0.0;
     if (nrm2 > 0.0) {
-        const double nrm = sqrt(nrm2);
-        beta = alpha >= 0.0 ? -nrm : nrm;
-        tau = (beta - alpha) / beta;
+        // one rsqrt and one reciprocal on the critical path (sqrt + two divisions cost 340 cycles on B200)
+        const double r = rsqrt(nrm2);
+        const double nrm = nrm2 * r;
+        const bool pos = alpha >= 0.0;
+        beta = pos ? -nrm : nrm;
+        tau = (beta - alpha) * (pos ? -r : r);
         scale = 1.0 / (alpha - beta);
     }
 }
@@ -158,6 +161,83 @@ __device__ void householder_form_q(double* X, int ld, int m, int kk, const doubl
         }
         __syncthreads();
     }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Group versions: the CTA is split into thread groups (multiples of a warp) that each factor their
+// own matrix and synchronise on their own named barrier, so two factorizations of one site run
+// side by side without meeting at a CTA-wide barrier.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void group_bar(int id, int nthreads) {
+    asm volatile("bar.sync %0, %1;" :: "r"(id), "r"(nthreads) : "memory");
+}
+
+// Householder QR of the m x n column-major X (leading dim ld) by a group of gn threads (thread gt of
+// the group; gn/4 >= n - 1 quads, m <= 4 * MAXK).  Same algorithm and output as householder_qr.
+template <int MAXK>
+__device__ void householder_qr_g(double* X, int ld, int m, int n, double* tau, int gt, int gn, int bar) {
+    const int kk = m < n ? m : n;
+    const int lane = gt & 31;
+    const int rg = lane & 3;
+    const unsigned qmask = 0xfu << (lane & ~3);
+    const int colidx = gt >> 2;
+    if (gt < 32) {     // reflector 0 (first warp of the group)
+        double ss = 0.0;
+        for (int i = lane; i < m; i += 32) { const double v = X[i]; ss = fma(v, v, ss); }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
+        double bet, t, scale;
+        reflector_from_norm(X[0], ss, bet, t, scale);
+        __syncwarp();
+        for (int i = 1 + lane; i < m; i += 32) X[i] *= scale;
+        if (lane == 0) { X[0] = bet; tau[0] = t; }
+    }
+    group_bar(bar, gn);
+    for (int j = 0; j < kk; ++j) {
+        const double* colj = X + (size_t)j * ld;
+        const double t = tau[j];
+        const int jj = j + 1 + colidx;
+        if (jj < n) {
+            double* col = X + (size_t)jj * ld;
+            double below2;
+            const double w = quad_dot_update<MAXK>(colj, col, j + 1, m, rg, qmask, t, col[j], below2);
+            if (rg == 0) col[j] -= w;
+            if (colidx == 0 && j + 1 < kk) {       // build reflector j+1 from the updated column
+                below2 += __shfl_xor_sync(qmask, below2, 1);
+                below2 += __shfl_xor_sync(qmask, below2, 2);
+                __syncwarp(qmask);
+                double bet, t1, scale;
+                reflector_from_norm(col[j + 1], below2, bet, t1, scale);
+                __syncwarp(qmask);
+                for (int i = j + 2 + rg; i < m; i += 4) col[i] *= scale;
+                if (rg == 0) { col[j + 1] = bet; tau[j + 1] = t1; }
+            }
+        }
+        group_bar(bar, gn);
+    }
+}
+
+// B <- Q B for the m x nb column-major B (leading dim ldb), Q = H_0 H_1 ... H_{kk-1} given by the
+// reflectors below the diagonal of V (leading dim ldv, unit diagonal implied) and tau, without ever
+// forming Q.  One quad per column of B (gn/4 >= nb); one group barrier per reflector.
+template <int MAXK>
+__device__ void householder_apply_g(const double* V, int ldv, const double* tau, int m, int kk,
+                                    double* B, int ldb, int nb, int gt, int gn, int bar) {
+    const int lane = gt & 31;
+    const int rg = lane & 3;
+    const unsigned qmask = 0xfu << (lane & ~3);
+    const int colidx = gt >> 2;
+    if (colidx < nb) {
+        double* col = B + (size_t)colidx * ldb;
+        for (int j = kk - 1; j >= 0; --j) {
+            double below2;
+            const double w = quad_dot_update<MAXK>(V + (size_t)j * ldv, col, j + 1, m, rg, qmask, tau[j], col[j], below2);
+            __syncwarp(qmask);
+            if (rg == 0) col[j] -= w;
+            __syncwarp(qmask);
+        }
+    }
+    (void)gn; (void)bar;
 }
 
 // Householder QR with column pivoting, R only:  X P = Q R  for the m x n column-major X in shared
