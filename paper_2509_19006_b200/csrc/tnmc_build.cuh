@@ -63,9 +63,9 @@ struct BuildCfg {
     static constexpr int Y_SZ = (D * LDM > LDX * D ? D * LDM : LDX * D);
     static constexpr int Z_OFF = Y_OFF + Y_SZ;            // D*D   : site tensor staging (QR sweep); M before rotation (SVD sweep)
     static constexpr int U_OFF = Z_OFF + D * D;           // D*LDU : C_a (QR sweep); carried Pc / M V_k (SVD sweep)
-    static constexpr int S_OFF = U_OFF + D * LDU;         // 3*D + 40 : tau / column norms / sigma / reduction scratch
-    static constexpr int N_DBL = S_OFF + 3 * D + 40;
-    static size_t smem_bytes(int L) { return sizeof(double) * N_DBL + sizeof(int) * (L + 2 + 2 * D); }
+    static constexpr int S_OFF = U_OFF + D * LDU;         // D + 24 + D + 40 : tau / QRCP scratch / sigma / reduction scratch
+    static constexpr int N_DBL = S_OFF + 2 * D + 64;
+    static size_t smem_bytes(int L) { return sizeof(double) * N_DBL + sizeof(int) * (L + 2 + 2 * D + 2); }
 };
 
 template <int P>
@@ -80,12 +80,13 @@ __global__ void __launch_bounds__(BuildCfg<P>::NT, 1) build_rows_kernel(const Bu
     double* sZ = smem + Cfg::Z_OFF;
     double* sU = smem + Cfg::U_OFF;
     double* sTau = smem + Cfg::S_OFF;    // [D]  tau of block a at a*P (QR sweep) / of the QRCP
-    double* sCn = sTau + D;              // [D]  remaining column norms of the QRCP
-    double* sSig = sCn + D;              // [D]  squared row norms of the Jacobi, then sigma
+    double* sCn = sTau + D;              // [24] per-warp (max, partial sum) scratch of the QRCP
+    double* sSig = sCn + 24;             // [D]  sigma
     double* sRed = sSig + D;             // [40] block reduction scratch
     int* sq = reinterpret_cast<int*>(smem + Cfg::N_DBL);   // [L+1] rows q_c of the carried R = left bond of Q_c
     int* spos = sq + args.L + 2;                           // [D] rank / position of each Jacobi row
-    int* sperm = spos + D;                                 // [D] column permutation of the QRCP
+    int* sperm = spos + D;                                 // [D] step at which each column was the QRCP pivot
+    int* sNr = sperm + D;                                  // [1] rows of R kept by the QRCP
 
     const int tid = threadIdx.x;
     const int half = tid >= HALF ? 1 : 0, gt = tid - half * HALF;
@@ -247,18 +248,20 @@ __global__ void __launch_bounds__(BuildCfg<P>::NT, 1) build_rows_kernel(const Bu
                 sM0[(size_t)col * D + x] = sX[(size_t)col * LDX + x];
             }
             PROF(7);
-            // M P = Q R with column pivoting (R only); the singular values and right singular vectors of
-            // M are those of R, with the columns permuted back
-            const double fro2 = householder_qrcp<MAXK>(sX, LDX, q, nc, sCn, sperm, sTau, nullptr);
-            const int nrow = q < nc ? q : nc;        // rows of R (even: q and nc are)
+            // M = Q (R P^T) with column pivoting, R only and in M's own column order; rows of R below the
+            // numerical rank (sigma <= 1e-15 |M|_F) are dropped.  Singular values and right singular
+            // vectors of M are those of R P^T.
+            int* spst = sperm;                       // step at which each column was the pivot
+            const double fro2 = householder_qrcp2<MAXK>(sX, LDX, q, nc, sCn, spos, spst, sNr);
+            const int nrow = *sNr;                   // rows of R kept (even)
             for (int t = tid; t < nrow * nc; t += NT) {
                 const int j = t % nc, i = t / nc;
-                sMj[(size_t)i * LDM + j] = j >= i ? sX[i + (size_t)j * LDX] : 0.0;
+                sMj[(size_t)i * LDM + j] = i <= spst[j] ? sX[i + (size_t)j * LDX] : 0.0;
             }
             __syncthreads();
             const double thr2 = fro2 * 1e-30;      // sigma <= 1e-15 |M|_F: below the numerical rank
             PROF(4);
-            const int nsw = jacobi_rows(sMj, LDM, nrow, nc, fro2, thr2, sSig, args.flags);
+            const int nsw = nrow >= 2 ? jacobi_rows2(sMj, LDM, nrow, nc, fro2, thr2, args.flags) : 0;
             PROF(5);
             PROF_ADD(8, nsw); PROF_ADD(9, 1);
             (void)nsw;
@@ -273,10 +276,14 @@ __global__ void __launch_bounds__(BuildCfg<P>::NT, 1) build_rows_kernel(const Bu
                     if (t8 == 0) sSig[x] = sqrt(a);
                 }
             }
-            for (int t = tid; t < TSZ; t += NT) stage[t] = 0.0;
-            __syncthreads();
             int k = chi < q ? chi : q;
             if (nc < k) k = nc;
+            for (int t = tid; t < TSZ; t += NT) stage[t] = 0.0;
+            if (k > nrow) {    // kept directions beyond the numerical rank stay zero rows
+                for (int t = tid; t < (k - nrow) * LDV; t += NT) sV[(size_t)nrow * LDV + t] = 0.0;
+                if (tid == 0) raise_flag(args.flags, FLAG_SIGMA_ZERO);
+            }
+            __syncthreads();
             for (int x = tid; x < nrow; x += NT) {
                 const double sx = sSig[x];
                 int rank = 0;
@@ -297,9 +304,8 @@ __global__ void __launch_bounds__(BuildCfg<P>::NT, 1) build_rows_kernel(const Bu
                     // a kept direction below the numerical rank carries no weight (M v = 0 for any
                     // orthonormal completion); it is stored as a zero row
                     const double v = sx * sx > thr2 ? sMj[(size_t)x * LDM + col] / sx : 0.0;
-                    const int oc = sperm[col];        // original column (a, y) of pivoted column col
-                    sV[(size_t)yp * LDV + oc] = v;
-                    stage[env_off(P, yp, oc / kprev, oc % kprev)] = v;
+                    sV[(size_t)yp * LDV + col] = v;     // col = (a, y) = a * kprev + y
+                    stage[env_off(P, yp, col / kprev, col % kprev)] = v;
                 }
             }
             __syncthreads();

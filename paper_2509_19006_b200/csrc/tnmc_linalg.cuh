@@ -313,6 +313,218 @@ __device__ double householder_qrcp(double* X, int ld, int m, int n, double* cn, 
     return fro2;
 }
 
+// Householder QR with column pivoting, R only, second version: one barrier per step, no column swaps.
+//   X (m x n, column-major, leading dim ld; m <= 4 MAXK, n <= blockDim/4) is overwritten by R in
+//   PHYSICAL column order: after the call, entry (i, col) of R P^T is X[i + col*ld] for
+//   i <= pstep[col] and 0 below (pstep[col] = step at which col was the pivot, or the number of
+//   steps done if it never was).  M = Q R P^T, so the rows of this matrix have the singular values
+//   and right singular vectors of M in M's own column coordinates -- nothing is permuted back.
+//   * Every quad owns a column and keeps its remaining squared norm, summed afresh inside every
+//     update (exact, no downdating).  Each warp reduces its columns to (max, index), writes the
+//     pair to shared memory, and after the step's single barrier every thread reads the <= 8 pairs
+//     and derives the same pivot and the same reflector scalars redundantly.
+//   * The reflector is never stored (R only): the pivot column is read as is and its scale is
+//     folded into the update, so the dot product runs beside the rsqrt/reciprocal chain.
+//   * Steps stop early (at an even step j) once (n - j) * max remaining norm^2 <= 1e-30 |X|_F^2:
+//     every further row of R is below the numerical rank (sigma <= 1e-15 |X|_F) and is dropped.
+//   wv / wi: >= 2 * 8 doubles / ints of scratch.  Returns |X|_F^2; *n_rows_out = rows of R kept (even).
+template <int MAXK>
+__device__ double householder_qrcp2(double* X, int ld, int m, int n, double* wv, int* wi, int* pstep, int* n_rows_out) {
+    const int kk = m < n ? m : n;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = blockDim.x >> 5;
+    const int rg = lane & 3;
+    const unsigned qmask = 0xfu << (lane & ~3);
+    const int cq = threadIdx.x >> 2;
+    const bool has_col = cq < n;
+    double* col = X + (size_t)(has_col ? cq : 0) * ld;
+    bool active = has_col;
+    double myn = -1.0;
+    if (has_col) {
+        double s0 = 0.0, s1 = 0.0;
+        for (int i = rg; i < m; i += 8) {
+            const double a = col[i]; s0 = fma(a, a, s0);
+            if (i + 4 < m) { const double b = col[i + 4]; s1 = fma(b, b, s1); }
+        }
+        double ss = s0 + s1;
+        ss += __shfl_xor_sync(qmask, ss, 1);
+        ss += __shfl_xor_sync(qmask, ss, 2);
+        myn = ss;
+    }
+    // |X|_F^2: per-warp partial sums (each column counted once, by its rg == 0 lane), fixed order
+    {
+        double part = (has_col && rg == 0) ? myn : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
+        if (lane == 0) wv[16 + warp] = part;
+    }
+    auto warp_argmax = [&](int buf) {
+        double bv = active ? myn : -1.0;
+        int bi = cq;
+#pragma unroll
+        for (int o = 4; o < 32; o <<= 1) {
+            const double ov = __shfl_xor_sync(0xffffffffu, bv, o);
+            const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+            if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
+        }
+        if (lane == 0) { wv[buf * 8 + warp] = bv; wi[buf * 8 + warp] = bi; }
+    };
+    warp_argmax(0);
+    __syncthreads();
+    double fro2 = 0.0;
+    for (int w = 0; w < nw; ++w) fro2 += wv[16 + w];
+    const double thr2 = fro2 * 1e-30;
+    int my_pstep = kk;
+    double pend_beta = 0.0;
+    int j = 0;
+    for (; j < kk; ++j) {
+        const int buf = j & 1;
+        double best = wv[buf * 8]; int bi = wi[buf * 8];
+        for (int w = 1; w < nw; ++w) {
+            const double ov = wv[buf * 8 + w]; const int oi = wi[buf * 8 + w];
+            if (ov > best || (ov == best && oi < bi)) { best = ov; bi = oi; }
+        }
+        if ((j & 1) == 0 && !(best * (double)(n - j) > thr2)) break;
+        const double* pc = X + (size_t)bi * ld;
+        double bet, tau, scale;
+        if (active && cq != bi) {
+            // dot product with the unscaled pivot column, beside the scalar chain
+            double x[MAXK], vv[MAXK];
+            double w0 = 0.0, w1 = 0.0;
+#pragma unroll
+            for (int k = 0; k < MAXK; ++k) {
+                const int i = j + 1 + rg + 4 * k;
+                const bool in = i < m;
+                x[k] = in ? col[i] : 0.0;
+                vv[k] = in ? pc[i] : 0.0;
+            }
+            const double cj = col[j];
+            reflector_from_norm(pc[j], best, bet, tau, scale);
+#pragma unroll
+            for (int k = 0; k < MAXK; k += 2) {
+                w0 = fma(vv[k], x[k], w0);
+                if (k + 1 < MAXK) w1 = fma(vv[k + 1], x[k + 1], w1);
+            }
+            double dot = w0 + w1;
+            dot += __shfl_xor_sync(qmask, dot, 1);
+            dot += __shfl_xor_sync(qmask, dot, 2);
+            const double w = tau * fma(scale, dot, cj);
+            const double ws = w * scale;
+            double s0 = 0.0, s1 = 0.0;
+#pragma unroll
+            for (int k = 0; k < MAXK; ++k) {
+                const int i = j + 1 + rg + 4 * k;
+                if (i < m) {
+                    const double nv = fma(-ws, vv[k], x[k]);
+                    col[i] = nv;
+                    if (k & 1) s1 = fma(nv, nv, s1); else s0 = fma(nv, nv, s0);
+                }
+            }
+            double below2 = s0 + s1;
+            below2 += __shfl_xor_sync(qmask, below2, 1);
+            below2 += __shfl_xor_sync(qmask, below2, 2);
+            if (rg == 0) col[j] = cj - w;
+            myn = below2;
+        } else if (active) {   // this quad owns the pivot: its column is final (row j becomes beta, written after the barrier)
+            reflector_from_norm(pc[j], best, bet, tau, scale);
+            pend_beta = bet;
+            my_pstep = j;
+            active = false;
+        }
+        warp_argmax(buf ^ 1);
+        __syncthreads();
+        if (my_pstep == j && has_col && rg == 0) col[j] = pend_beta;
+    }
+    if (has_col && rg == 0) pstep[cq] = my_pstep < j ? my_pstep : j;
+    *n_rows_out = j;
+    __syncthreads();
+    return fro2;
+}
+
+// One-sided (Hestenes) Jacobi on the rows of M, second version: as jacobi_rows, but a pair's two
+// squared norms are summed together with its dot product from the registers that hold the rows
+// (three sums share the three shuffle stages), so nothing is cached in shared memory, nothing is
+// updated after a rotation and nothing is refreshed per sweep; and the rotation comes from two FP64
+// rsqrt with no division and no FP32 detour:
+//   d = b - a, h = sqrt(d^2 + 4 g^2), u = |d| + h, w = 1 / sqrt(u^2 + 4 g^2), cos = u w, sin = sign(d) 2 g w.
+// All n rows take part (n even); rows at or below thr2 are left alone.  Returns the sweeps done.
+__device__ int jacobi_rows2(double* M, int ld, int n, int nc, double fro2, double thr2, unsigned long long* flags) {
+    const int grp = threadIdx.x >> 3, t8 = threadIdx.x & 7;
+    const int npairs = n >> 1;
+    const unsigned gmask = 0xffu << ((threadIdx.x & 31) & ~7);
+    const double rot2 = 256.0 * 4.930380657631324e-32;             // (16 eps)^2
+    const double big2 = 1e-16;                                     // (1e-8)^2
+    const double floor2 = 65536.0 * 4.930380657631324e-32 * fro2;  // (256 eps |M|_F)^2
+    const int c0 = 2 * t8;                                         // this lane's columns: c0 + 16 k, c0 + 16 k + 1
+    int sweep = 0;
+    for (; sweep < 60; ++sweep) {
+        int big = 0;
+        for (int round = 0; round < n - 1; ++round) {
+            if (grp < npairs) {
+                int r1, r2;
+                if (grp == 0) { r1 = n - 1; r2 = round; }
+                else {
+                    r1 = round + grp; if (r1 >= n - 1) r1 -= n - 1;
+                    r2 = round - grp; if (r2 < 0) r2 += n - 1;
+                }
+                if (r1 > r2) { const int t = r1; r1 = r2; r2 = t; }
+                double* x = M + (size_t)r1 * ld;
+                double* y = M + (size_t)r2 * ld;
+                double2 xv[4], yv[4];
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const int c = c0 + 16 * k;
+                    if (c < nc) {
+                        xv[k] = *reinterpret_cast<const double2*>(x + c);
+                        yv[k] = *reinterpret_cast<const double2*>(y + c);
+                    } else { xv[k] = make_double2(0.0, 0.0); yv[k] = make_double2(0.0, 0.0); }
+                }
+                double a = 0.0, b = 0.0, g = 0.0, a1 = 0.0, b1 = 0.0, g1 = 0.0;
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    a = fma(xv[k].x, xv[k].x, a);  a1 = fma(xv[k].y, xv[k].y, a1);
+                    b = fma(yv[k].x, yv[k].x, b);  b1 = fma(yv[k].y, yv[k].y, b1);
+                    g = fma(xv[k].x, yv[k].x, g);  g1 = fma(xv[k].y, yv[k].y, g1);
+                }
+                a += a1; b += b1; g += g1;
+#pragma unroll
+                for (int o = 4; o > 0; o >>= 1) {
+                    a += __shfl_xor_sync(gmask, a, o);
+                    b += __shfl_xor_sync(gmask, b, o);
+                    g += __shfl_xor_sync(gmask, g, o);
+                }
+                const double g2 = g * g, ab = a * b;
+                if (a > thr2 && b > thr2 && g2 > rot2 * ab) {
+                    const double mx = a > b ? a : b;
+                    big |= (g2 > big2 * ab) && (g2 > floor2 * mx);
+                    const double dd = b - a;
+                    const double g24 = 4.0 * g2;
+                    const double h2 = fma(dd, dd, g24);
+                    const double u = fabs(dd) + h2 * rsqrt(h2);
+                    const double w = rsqrt(fma(u, u, g24));
+                    const double cs = u * w;
+                    double sn = 2.0 * g * w;
+                    if (dd < 0.0) sn = -sn;
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) {
+                        const int c = c0 + 16 * k;
+                        if (c < nc) {
+                            double2 xn, yn;
+                            xn.x = fma(cs, xv[k].x, -sn * yv[k].x);  yn.x = fma(sn, xv[k].x, cs * yv[k].x);
+                            xn.y = fma(cs, xv[k].y, -sn * yv[k].y);  yn.y = fma(sn, xv[k].y, cs * yv[k].y);
+                            *reinterpret_cast<double2*>(x + c) = xn;
+                            *reinterpret_cast<double2*>(y + c) = yn;
+                        }
+                    }
+                }
+            }
+            __syncthreads();
+        }
+        if (!__syncthreads_or(big)) { ++sweep; break; }
+    }
+    if (sweep >= 60 && threadIdx.x == 0) raise_flag(flags, FLAG_JACOBI_LIMIT);
+    return sweep;
+}
+
 // One-sided (Hestenes) Jacobi on the ROWS of the n x nc row-major matrix M (row length ld, a
 // multiple of 2; nc <= 64): plane rotations from the left until all rows are mutually orthogonal,
 // so that row x ends as sigma_x * v_x^T (M = U Sigma V^T).  n must be even.
