@@ -113,6 +113,7 @@ static tnmc_status launch_build(tnmc_ctx* ctx, int m, int row_hi, int row_lo, in
     a.slot_of_row = ctx->map(m);
     a.env = ctx->at<double>(p.off_env); a.env_dis_stride = p.env_dis_stride;
     a.qbuf = ctx->at<double>(p.off_qbuf);
+    a.m0buf = ctx->at<double>(p.off_m0);
     a.logscale = ctx->at<double>(p.off_logscale);
     a.flags = ctx->at<unsigned long long>(p.off_flags);
     cudaError_t e;

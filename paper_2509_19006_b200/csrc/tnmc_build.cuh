@@ -42,6 +42,7 @@ struct BuildArgs {
     double* env;                 // env base
     size_t env_dis_stride;       // doubles per disorder (n_slots * L * 2P^2)
     double* qbuf;                // scratch, per disorder L * QSZ doubles (reflectors of the QR sweep)
+    double* m0buf;               // scratch, per disorder D*D doubles (M before rotation; used when P == 32)
     double* logscale;            // (n_dis, L): logscale of every row (written for rows built)
     unsigned long long* flags;
 };
@@ -61,15 +62,19 @@ struct BuildCfg {
     static constexpr int X_OFF = 0;                       // LDX*D : T_0 | T_1 (QR sweep); M, then stage + V_k (SVD sweep)
     static constexpr int Y_OFF = X_OFF + LDX * D;         // D*LDM >= 2*D*LDR, LDX*D : carried R (QR sweep); reflectors, then Jacobi operand
     static constexpr int Y_SZ = (D * LDM > LDX * D ? D * LDM : LDX * D);
-    static constexpr int Z_OFF = Y_OFF + Y_SZ;            // D*D   : site tensor staging (QR sweep); M before rotation (SVD sweep)
-    static constexpr int U_OFF = Z_OFF + D * D;           // D*LDU : C_a (QR sweep); carried Pc / M V_k (SVD sweep)
+    // M before rotation (needed once more for M V_k) lives in shared memory for P <= 16 and in an
+    // L2-resident global scratch for P = 32, which brings the CTA to 88 KB: two CTAs per SM.
+    static constexpr bool M0_GLOBAL = P >= 32;
+    static constexpr int CTAS_PER_SM = P >= 32 ? 2 : 3;
+    static constexpr int Z_OFF = Y_OFF + Y_SZ;            // D*D   : M before rotation (SVD sweep), P <= 16 only
+    static constexpr int U_OFF = Z_OFF + (M0_GLOBAL ? 0 : D * D);   // D*LDU : C_a (QR sweep); carried Pc / M V_k (SVD sweep)
     static constexpr int S_OFF = U_OFF + D * LDU;         // D + 24 + D + 40 : tau / QRCP scratch / sigma / reduction scratch
     static constexpr int N_DBL = S_OFF + 2 * D + 64;
     static size_t smem_bytes(int L) { return sizeof(double) * N_DBL + sizeof(int) * (L + 2 + 2 * D + 2); }
 };
 
 template <int P>
-__global__ void __launch_bounds__(BuildCfg<P>::NT, 1) build_rows_kernel(const BuildArgs args) {
+__global__ void __launch_bounds__(BuildCfg<P>::NT, BuildCfg<P>::CTAS_PER_SM) build_rows_kernel(const BuildArgs args) {
     using Cfg = BuildCfg<P>;
     constexpr int NT = Cfg::NT, HALF = NT / 2, D = Cfg::D, LDX = Cfg::LDX, LDM = Cfg::LDM, LDV = Cfg::LDV,
                   LDR = Cfg::LDR, LDU = Cfg::LDU, TSZ = Cfg::TSZ;
@@ -77,7 +82,7 @@ __global__ void __launch_bounds__(BuildCfg<P>::NT, 1) build_rows_kernel(const Bu
     extern __shared__ __align__(16) double smem[];
     double* sX = smem + Cfg::X_OFF;
     double* sY = smem + Cfg::Y_OFF;
-    double* sZ = smem + Cfg::Z_OFF;
+    double* sA = sX;                     // site tensor staging of the QR sweep (X is free until T is written)
     double* sU = smem + Cfg::U_OFF;
     double* sTau = smem + Cfg::S_OFF;    // [D]  tau of block a at a*P (QR sweep) / of the QRCP
     double* sCn = sTau + D;              // [24] per-warp (max, partial sum) scratch of the QRCP
@@ -111,14 +116,14 @@ __global__ void __launch_bounds__(BuildCfg<P>::NT, 1) build_rows_kernel(const Bu
             const int bl = row_bond(L, chi, r + 1, c), br = row_bond(L, chi, r + 1, c + 1);
             const int q = sq[c];
             const double* Ain = env_in + (size_t)c * TSZ;
-            for (int t = tid; t < TSZ; t += NT) sZ[t] = Ain[t];
+            for (int t = tid; t < TSZ; t += NT) sA[t] = Ain[t];
             __syncthreads();
             {   // C_a[i][k] = sum_m B_d[a][m] A[i][m][k]      (Eq. 7: B_d[a][m] = exp(beta Jd (2a-1)(2m-1)))
                 const int jd = args.J.jd(d, r, c);
                 const double w_same = exp(beta * jd), w_diff = exp(-beta * jd);
                 for (int t = tid; t < 2 * bl * br; t += NT) {
                     const int k = t % br, i = (t / br) % bl, a = t / (br * bl);
-                    sU[(a * P + i) * LDU + k] = w_same * sZ[env_off(P, i, a, k)] + w_diff * sZ[env_off(P, i, 1 - a, k)];
+                    sU[(a * P + i) * LDU + k] = w_same * sA[env_off(P, i, a, k)] + w_diff * sA[env_off(P, i, 1 - a, k)];
                 }
             }
             __syncthreads();
@@ -189,7 +194,7 @@ __global__ void __launch_bounds__(BuildCfg<P>::NT, 1) build_rows_kernel(const Bu
 
         // ------------------------------------------------------------------ B. SVD sweep, right -> left
         double* sMj = sY;             // Jacobi operand (rows of R), row-major, row length LDM
-        double* sM0 = sZ;             // M before rotation, column-major, leading dim D
+        double* sM0 = Cfg::M0_GLOBAL ? args.m0buf + (size_t)d * D * D : smem + Cfg::Z_OFF;   // M before rotation, column-major, leading dim D
         double* stage = sX;           // output tensor in fragment order (once the QRCP result has left X)
         double* sV = sX + TSZ;        // [y'][col], row length LDV: selected right singular vectors
         int kprev = 1;
@@ -261,7 +266,7 @@ __global__ void __launch_bounds__(BuildCfg<P>::NT, 1) build_rows_kernel(const Bu
             __syncthreads();
             const double thr2 = fro2 * 1e-30;      // sigma <= 1e-15 |M|_F: below the numerical rank
             PROF(4);
-            const int nsw = nrow >= 2 ? jacobi_rows2(sMj, LDM, nrow, nc, fro2, thr2, args.flags) : 0;
+            const int nsw = nrow >= 2 ? jacobi_rows2<(D + 15) / 16>(sMj, LDM, nrow, nc, fro2, thr2, args.flags) : 0;
             PROF(5);
             PROF_ADD(8, nsw); PROF_ADD(9, 1);
             (void)nsw;

@@ -28,7 +28,7 @@ struct Plan {
     size_t qsz = 0;                 // doubles per site of the Q scratch
     // byte offsets into the workspace
     size_t off_masks = 0, off_maps = 0, off_flags = 0, off_logscale = 0, off_logz = 0, off_env = 0,
-           off_qbuf = 0, off_renv = 0, total = 0;
+           off_qbuf = 0, off_m0 = 0, off_renv = 0, total = 0;
 
     int ckpt_slot(int j) const { return j; }
     int bottom_slot() const { return n_seg; }
@@ -83,6 +83,7 @@ inline bool make_plan(Plan& p, int L, int chi, int n_dis, int n_samples_max, int
     p.off_logz = o;     o = align_up(o + sizeof(double) * (size_t)n_dis);
     p.off_env = o;      o = align_up(o + sizeof(double) * (size_t)n_dis * p.env_dis_stride);
     p.off_qbuf = o;     o = align_up(o + sizeof(double) * (size_t)n_dis * L * p.qsz);
+    p.off_m0 = o;       o = align_up(o + sizeof(double) * (size_t)n_dis * 4 * p.P * p.P);
     p.off_renv = o;     o = align_up(o + sizeof(double) * (size_t)n_dis * p.tiles * L * SAMPLE_CHAINS * p.P);
     p.total = o;
     return true;

@@ -446,7 +446,9 @@ __device__ double householder_qrcp2(double* X, int ld, int m, int n, double* wv,
 // updated after a rotation and nothing is refreshed per sweep; and the rotation comes from two FP64
 // rsqrt with no division and no FP32 detour:
 //   d = b - a, h = sqrt(d^2 + 4 g^2), u = |d| + h, w = 1 / sqrt(u^2 + 4 g^2), cos = u w, sin = sign(d) 2 g w.
-// All n rows take part (n even); rows at or below thr2 are left alone.  Returns the sweeps done.
+// All n rows take part (n even); rows at or below thr2 are left alone.  NK = ceil(max nc / 16)
+// column pairs per lane.  Returns the sweeps done.
+template <int NK>
 __device__ int jacobi_rows2(double* M, int ld, int n, int nc, double fro2, double thr2, unsigned long long* flags) {
     const int grp = threadIdx.x >> 3, t8 = threadIdx.x & 7;
     const int npairs = n >> 1;
@@ -469,9 +471,9 @@ __device__ int jacobi_rows2(double* M, int ld, int n, int nc, double fro2, doubl
                 if (r1 > r2) { const int t = r1; r1 = r2; r2 = t; }
                 double* x = M + (size_t)r1 * ld;
                 double* y = M + (size_t)r2 * ld;
-                double2 xv[4], yv[4];
+                double2 xv[NK], yv[NK];
 #pragma unroll
-                for (int k = 0; k < 4; ++k) {
+                for (int k = 0; k < NK; ++k) {
                     const int c = c0 + 16 * k;
                     if (c < nc) {
                         xv[k] = *reinterpret_cast<const double2*>(x + c);
@@ -480,7 +482,7 @@ __device__ int jacobi_rows2(double* M, int ld, int n, int nc, double fro2, doubl
                 }
                 double a = 0.0, b = 0.0, g = 0.0, a1 = 0.0, b1 = 0.0, g1 = 0.0;
 #pragma unroll
-                for (int k = 0; k < 4; ++k) {
+                for (int k = 0; k < NK; ++k) {
                     a = fma(xv[k].x, xv[k].x, a);  a1 = fma(xv[k].y, xv[k].y, a1);
                     b = fma(yv[k].x, yv[k].x, b);  b1 = fma(yv[k].y, yv[k].y, b1);
                     g = fma(xv[k].x, yv[k].x, g);  g1 = fma(xv[k].y, yv[k].y, g1);
@@ -505,7 +507,7 @@ __device__ int jacobi_rows2(double* M, int ld, int n, int nc, double fro2, doubl
                     double sn = 2.0 * g * w;
                     if (dd < 0.0) sn = -sn;
 #pragma unroll
-                    for (int k = 0; k < 4; ++k) {
+                    for (int k = 0; k < NK; ++k) {
                         const int c = c0 + 16 * k;
                         if (c < nc) {
                             double2 xn, yn;
