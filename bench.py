@@ -205,37 +205,55 @@ def main_ours(args):
     Jr, Jd = Jr_h.to(dev), Jd_h.to(dev)
     need = tnmc.tnmc_workspace_bytes(L, chi, n_dis, n_s, ckpt_stride=ckpt)
     need_h = tnmc.tnmc_run_host_workspace_bytes(L, chi, n_dis, n_s, ckpt_stride=ckpt)
-    ws = torch.empty(max(need, need_h), dtype=torch.uint8, device=dev)
     W = tnmc.words(L)
-    bits = torch.empty((n_dis, n_s, L, W), dtype=torch.int32, device=dev)
-    logq = torch.empty((n_dis, n_s), dtype=torch.float64, device=dev)
-    E = torch.empty((n_dis, n_s), dtype=torch.int32, device=dev)
-    logZ = torch.empty(n_dis, dtype=torch.float64, device=dev)
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
+    nb = len(betas)
+    # the betas of a step are independent problems: each gets its own stream, workspace and outputs, and
+    # the nb launches of every phase run side by side (fork/join on events around each phase)
     stream = torch.cuda.current_stream()
+    streams = [stream] + [torch.cuda.Stream(device=dev) for _ in range(nb - 1)]
+    ws = [torch.empty(max(need, need_h), dtype=torch.uint8, device=dev) for _ in betas]
+    bits = [torch.empty((n_dis, n_s, L, W), dtype=torch.int32, device=dev) for _ in betas]
+    logq = [torch.empty((n_dis, n_s), dtype=torch.float64, device=dev) for _ in betas]
+    E = [torch.empty((n_dis, n_s), dtype=torch.int32, device=dev) for _ in betas]
+    logZ = [torch.empty(n_dis, dtype=torch.float64, device=dev) for _ in betas]
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
     ev = lambda: torch.cuda.Event(enable_timing=True)
+    PHASES = ("build", "sample", "energy", "metropolis")
 
     def step(timed):
         """one pass over the batch; returns (accepted, launches, phase ms dict)"""
-        acc, launches = 0, 0
-        ph = {"build": 0.0, "sample": 0.0, "energy": 0.0, "metropolis": 0.0}
-        evs = []
-        for beta in betas:
-            ctx = tnmc.Context(L, chi, beta, Jr, Jd, n_s, first_disorder=first, ckpt_stride=ckpt, workspace=ws)
-            e = [ev() for _ in range(5)]
-            e[0].record(stream); ctx.tnmc_build_envs(logZ)
-            e[1].record(stream); ctx.tnmc_sample(n_s, c["seed"], cfg_bits=bits, logq=logq)
-            e[2].record(stream); ctx.tnmc_energy(bits, E=E)
-            e[3].record(stream); _, n_acc, _, _ = ctx.tnmc_metropolis(E, logq, c["seed"])
-            e[4].record(stream)
-            evs.append((e, n_acc, ctx))
+        ctxs, n_accs = [None] * nb, [None] * nb
+
+        def run(phase, i):
+            if phase == "build":
+                ctxs[i] = tnmc.Context(L, chi, betas[i], Jr, Jd, n_s, first_disorder=first, ckpt_stride=ckpt, workspace=ws[i])
+                ctxs[i].tnmc_build_envs(logZ[i])
+            elif phase == "sample":
+                ctxs[i].tnmc_sample(n_s, c["seed"], cfg_bits=bits[i], logq=logq[i])
+            elif phase == "energy":
+                ctxs[i].tnmc_energy(bits[i], E=E[i])
+            else:
+                _, n_accs[i], _, _ = ctxs[i].tnmc_metropolis(E[i], logq[i], c["seed"])
+
+        e = [ev() for _ in range(len(PHASES) + 1)]
+        e[0].record(stream)
+        for k, phase in enumerate(PHASES):
+            for i, s in enumerate(streams):
+                if i > 0:
+                    s.wait_event(e[k])
+                with torch.cuda.stream(s):
+                    run(phase, i)
+            for s in streams[1:]:
+                done = torch.cuda.Event()
+                done.record(s)
+                stream.wait_event(done)
+            e[k + 1].record(stream)
         torch.cuda.synchronize()
-        for e, n_acc, ctx in evs:
-            acc += int(n_acc.sum().item())
-            launches += ctx.tnmc_launch_count()
-            for i, k in enumerate(ph):
-                ph[k] += e[i].elapsed_time(e[i + 1])
-            ctx.close()
+        acc = sum(int(n.sum().item()) for n in n_accs)
+        launches = sum(cx.tnmc_launch_count() for cx in ctxs)
+        ph = {k: e[i].elapsed_time(e[i + 1]) for i, k in enumerate(PHASES)}
+        for cx in ctxs:
+            cx.close()
         return acc, launches, ph
 
     def barrier():
@@ -269,36 +287,43 @@ def main_ours(args):
     ms_total, acc_total = t.item(), a.item()
     value = acc_total / (ms_total * 1e-3)
 
-    # ---- end to end: host buffers through tnmc_run_host
+    # ---- end to end: host buffers through tnmc_run_host, one host thread + stream per beta
     e2e = None
     if not args.no_e2e:
-        outs = None
-        for _ in range(2):
-            for beta in betas:
-                outs = tnmc.tnmc_run_host(L, chi, beta, Jr_h, Jd_h, n_s, c["seed"], ws, first_disorder=first, ckpt_stride=ckpt, out=outs)
-        e_acc, t0 = 0, None
-        barrier()
-        t0 = time.perf_counter()
-        for _ in range(args.steps):
-            for beta in betas:
-                outs = tnmc.tnmc_run_host(L, chi, beta, Jr_h, Jd_h, n_s, c["seed"], ws, first_disorder=first, ckpt_stride=ckpt, out=outs)
-                e_acc += int(outs["n_accepted"].sum().item())
-        torch.cuda.synchronize()
-        dt = time.perf_counter() - t0
+        from concurrent.futures import ThreadPoolExecutor
+        outs = [None] * nb
+
+        def host_pass(i):
+            torch.cuda.set_device(local_rank)
+            with torch.cuda.stream(streams[i]):
+                outs[i] = tnmc.tnmc_run_host(L, chi, betas[i], Jr_h, Jd_h, n_s, c["seed"], ws[i], first_disorder=first,
+                                             ckpt_stride=ckpt, out=outs[i])
+            return int(outs[i]["n_accepted"].sum().item())
+
+        with ThreadPoolExecutor(max_workers=nb) as pool:
+            for _ in range(2):
+                list(pool.map(host_pass, range(nb)))
+            e_acc = 0
+            barrier()
+            t0 = time.perf_counter()
+            for _ in range(args.steps):
+                e_acc += sum(pool.map(host_pass, range(nb)))
+            torch.cuda.synchronize()
+            dt = time.perf_counter() - t0
         te = torch.tensor([dt], dtype=torch.float64, device=dev)
         ae = torch.tensor([float(e_acc)], dtype=torch.float64, device=dev)
         if world > 1:
             dist.all_reduce(te, op=dist.ReduceOp.MAX)
             dist.all_reduce(ae, op=dist.ReduceOp.SUM)
-        h2d = len(betas) * (Jr_h.numel() + Jd_h.numel())
-        d2h = len(betas) * sum(v.numel() * v.element_size() for v in outs.values() if v is not None)
+        h2d = nb * (Jr_h.numel() + Jd_h.numel())
+        d2h = sum(v.numel() * v.element_size() for o in outs for v in o.values() if v is not None)
         e2e = {"value": ae.item() / te.item(), "unit": "samples/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h}
 
     if rank == 0:
-        nb = len(betas) * args.steps
-        build_ms = phases["build"] / nb                      # average duration of one tnmc_build_envs (one build_rows_kernel launch)
-        sample_ms = phases["sample"] / nb
-        build_flops = model.build_flops_per_disorder(L, chi) * n_dis * (2.0 if ckpt else 1.0)
+        # the nb launches of a phase run concurrently: duration of the group, algorithmic work of the group
+        build_ms = phases["build"] / args.steps
+        sample_ms = phases["sample"] / args.steps
+        build_flops = nb * model.build_flops_per_disorder(L, chi) * n_dis * (2.0 if ckpt else 1.0)
         peak_dmma = tnmc.tnmc_fp64_peak_tflops(1)
         peak_dfma = tnmc.tnmc_fp64_peak_tflops(0)
         peaks = {}
@@ -307,19 +332,19 @@ def main_ours(args):
         except Exception:
             pass
         hbm_peak = peaks.get("hbm_gbs", 6650.0)
-        samp_flops = model.sample_flops_per_chain_site(P) * n_dis * n_s * L * L
-        samp_bytes = model.sample_bytes_per_chain_site(P) * n_dis * n_s * L * L
+        samp_flops = nb * model.sample_flops_per_chain_site(P) * n_dis * n_s * L * L
+        samp_bytes = nb * model.sample_bytes_per_chain_site(P) * n_dis * n_s * L * L
         dominant = "build_rows_kernel" if phases["build"] >= phases["sample"] else "sample_rows_kernel"
         if dominant == "build_rows_kernel":
             ach = build_flops / (build_ms * 1e-3) / 1e12
             roof = {"bound": "alu", "kernel": dominant, "achieved": ach, "peak": peak_dfma, "unit": "TFLOP/s", "frac": ach / peak_dfma,
                     "traffic": None, "peak_source": "FP64 DFMA rate measured live by tnmc_fp64_peak_tflops(0) on this GPU",
-                    "algorithmic_flops_per_launch": build_flops}
+                    "algorithmic_flops_per_launch_group": build_flops, "launches_per_group": nb}
         else:
             ach = samp_flops / (sample_ms * 1e-3) / 1e12
             roof = {"bound": "tensor", "kernel": dominant, "achieved": ach, "peak": peak_dmma, "unit": "TFLOP/s", "frac": ach / peak_dmma,
                     "traffic": None, "peak_source": "FP64 DMMA (mma.sync.m8n8k4.f64) rate measured live by tnmc_fp64_peak_tflops(1)",
-                    "algorithmic_flops_per_launch": samp_flops}
+                    "algorithmic_flops_per_launch_group": samp_flops, "launches_per_group": nb}
         roof["other_kernels"] = {
             "sample_rows_kernel": {"ms": sample_ms, "tflops": samp_flops / (sample_ms * 1e-3) / 1e12, "frac_dmma_peak": samp_flops / (sample_ms * 1e-3) / 1e12 / peak_dmma,
                                    "hbm_gbs": samp_bytes / (sample_ms * 1e-3) / 1e9, "frac_hbm_peak": samp_bytes / (sample_ms * 1e-3) / 1e9 / hbm_peak},
@@ -337,7 +362,8 @@ def main_ours(args):
                 "vs_baseline": None, "dtype": "f64", "data": "synthetic",
                 "config": {"workload": args.workload, "note": c["note"], "L": L, "chi": chi, "betas": betas, "n_dis_per_gpu": n_dis,
                            "n_samples": n_s, "ckpt_stride": ckpt, "parallelism": f"dp{world} (disorders sharded, no collective)",
-                           "l2": "flushed (256 MiB memset) between timed steps; env stack > L2"},
+                           "l2": "flushed (256 MiB memset) between timed steps; env stack > L2",
+                           "streams": f"{nb} (one per beta; the launches of each phase run concurrently)"},
                 "proposals_per_s": len(betas) * args.steps * n_dis * n_s * world / (ms_total * 1e-3),
                 "p_acc": acc_total / (len(betas) * args.steps * n_dis * (n_s - 1) * world),
                 "phase_ms_per_step": {k: v / args.steps for k, v in phases.items()},
