@@ -69,8 +69,8 @@ struct BuildCfg {
     static constexpr int Z_OFF = Y_OFF + Y_SZ;            // D*D   : M before rotation (SVD sweep), P <= 16 only
     static constexpr int U_OFF = Z_OFF + (M0_GLOBAL ? 0 : D * D);   // D*LDU : C_a (QR sweep); carried Pc / M V_k (SVD sweep)
     static constexpr int S_OFF = U_OFF + D * LDU;         // D + 24 + D + 40 : tau / QRCP scratch / sigma / reduction scratch
-    static constexpr int N_DBL = S_OFF + 2 * D + 64;
-    static size_t smem_bytes(int L) { return sizeof(double) * N_DBL + sizeof(int) * (L + 2 + 2 * D + 2); }
+    static constexpr int N_DBL = S_OFF + 2 * D + 64 + 48 + 40;
+    static size_t smem_bytes(int L) { return sizeof(double) * N_DBL + sizeof(int) * (L + 2 + 2 * D + 2 + 48); }
 };
 
 template <int P>
@@ -85,13 +85,14 @@ __global__ void __launch_bounds__(BuildCfg<P>::NT, BuildCfg<P>::CTAS_PER_SM) bui
     double* sA = sX;                     // site tensor staging of the QR sweep (X is free until T is written)
     double* sU = smem + Cfg::U_OFF;
     double* sTau = smem + Cfg::S_OFF;    // [D]  tau of block a at a*P (QR sweep) / of the QRCP
-    double* sCn = sTau + D;              // [24] per-warp (max, partial sum) scratch of the QRCP
-    double* sSig = sCn + 24;             // [D]  sigma
+    double* sCn = sTau + D;              // [64 + 8] remaining column norms and per-warp partial sums of the QRCP
+    double* sSig = sCn + 72;             // [D]  sigma
     double* sRed = sSig + D;             // [40] block reduction scratch
     int* sq = reinterpret_cast<int*>(smem + Cfg::N_DBL);   // [L+1] rows q_c of the carried R = left bond of Q_c
     int* spos = sq + args.L + 2;                           // [D] rank / position of each Jacobi row
     int* sperm = spos + D;                                 // [D] step at which each column was the QRCP pivot
-    int* sNr = sperm + D;                                  // [1] rows of R kept by the QRCP
+    int* sNr = sperm + D;                                  // [2] rows of R kept by the QRCP
+    unsigned* sWk = reinterpret_cast<unsigned*>(sNr + 2);  // [48] per-warp pivot candidates of the QRCP
 
     const int tid = threadIdx.x;
     const int half = tid >= HALF ? 1 : 0, gt = tid - half * HALF;
@@ -257,7 +258,7 @@ __global__ void __launch_bounds__(BuildCfg<P>::NT, BuildCfg<P>::CTAS_PER_SM) bui
             // numerical rank (sigma <= 1e-15 |M|_F) are dropped.  Singular values and right singular
             // vectors of M are those of R P^T.
             int* spst = sperm;                       // step at which each column was the pivot
-            const double fro2 = householder_qrcp2<MAXK>(sX, LDX, q, nc, sCn, spos, spst, sNr);
+            const double fro2 = householder_qrcp2<MAXK>(sX, LDX, q, nc, sCn, sWk, spst, sNr);
             const int nrow = *sNr;                   // rows of R kept (even)
             for (int t = tid; t < nrow * nc; t += NT) {
                 const int j = t % nc, i = t / nc;

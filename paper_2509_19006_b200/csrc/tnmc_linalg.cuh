@@ -27,6 +27,32 @@ __device__ __forceinline__ double block_sum(double v, double* scratch) {
     return t;
 }
 
+// 1/sqrt(x) and 1/x for normal positive-range doubles without the library routines' special-case
+// handling: the MUFU seed (relative error <= 2^-22) and two Newton steps (error squared each time,
+// ~1 ulp at the end).  x must be finite, normal and (for rsqrt) positive -- true for every squared
+// norm and pivot that reaches them (zeros are excluded by the callers).
+__device__ __forceinline__ double fast_rsqrt(double x) {
+#ifdef TNMC_SLOW_MATH
+    return rsqrt(x);
+#endif
+    double r;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    const double hx = 0.5 * x;
+    r = r * fma(-hx * r, r, 1.5);
+    r = r * fma(-hx * r, r, 1.5);
+    return r;
+}
+__device__ __forceinline__ double fast_rcp(double x) {
+#ifdef TNMC_SLOW_MATH
+    return 1.0 / x;
+#endif
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    r = fma(r, fma(-x, r, 1.0), r);
+    r = fma(r, fma(-x, r, 1.0), r);
+    return r;
+}
+
 // Quad-cooperative column kernels used by the Householder routines.  A quad (4 lanes, rg = lane & 3)
 // owns one column; lane rg handles rows i0 + rg + 4k.  MAXK = max rows per lane.  Loads are batched
 // into registers (independent accumulators) so that shared-memory latency overlaps.
@@ -73,14 +99,14 @@ __device__ __forceinline__ double quad_dot_update(const double* __restrict__ v, 
 // cancellation): beta = -sign(alpha) sqrt(nrm2), tau = (beta - alpha) / beta, v_i = x_i / (alpha - beta).
 __device__ __forceinline__ void reflector_from_norm(double alpha, double nrm2, double& beta, double& tau, double& scale) {
     beta = alpha; tau = 0.0; scale = 0.0;
-    if (nrm2 > 0.0) {
+    if (nrm2 > 1e-280) {   // (smaller: the column is numerically zero against anything it could matter to)
         // one rsqrt and one reciprocal on the critical path (sqrt + two divisions cost 340 cycles on B200)
-        const double r = rsqrt(nrm2);
+        const double r = fast_rsqrt(nrm2);
         const double nrm = nrm2 * r;
         const bool pos = alpha >= 0.0;
         beta = pos ? -nrm : nrm;
         tau = (beta - alpha) * (pos ? -r : r);
-        scale = 1.0 / (alpha - beta);
+        scale = fast_rcp(alpha - beta);
     }
 }
 
@@ -327,9 +353,10 @@ __device__ double householder_qrcp(double* X, int ld, int m, int n, double* cn, 
 //     folded into the update, so the dot product runs beside the rsqrt/reciprocal chain.
 //   * Steps stop early (at an even step j) once (n - j) * max remaining norm^2 <= 1e-30 |X|_F^2:
 //     every further row of R is below the numerical rank (sigma <= 1e-15 |X|_F) and is dropped.
-//   wv / wi: >= 2 * 8 doubles / ints of scratch.  Returns |X|_F^2; *n_rows_out = rows of R kept (even).
+//   Returns |X|_F^2; *n_rows_out = rows of R kept (even).
 template <int MAXK>
-__device__ double householder_qrcp2(double* X, int ld, int m, int n, double* wv, int* wi, int* pstep, int* n_rows_out) {
+__device__ double householder_qrcp2(double* X, int ld, int m, int n, double* cn, unsigned* wk, int* pstep, int* n_rows_out) {
+    // cn: [8] per-warp partial sums at cn + 64;  wk: [2][3][8] per-warp (norm pattern high, low, column)
     const int kk = m < n ? m : n;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = blockDim.x >> 5;
     const int rg = lane & 3;
@@ -337,8 +364,9 @@ __device__ double householder_qrcp2(double* X, int ld, int m, int n, double* wv,
     const int cq = threadIdx.x >> 2;
     const bool has_col = cq < n;
     double* col = X + (size_t)(has_col ? cq : 0) * ld;
+    double* wsum = cn + 64;
     bool active = has_col;
-    double myn = -1.0;
+    double myn = 0.0;
     if (has_col) {
         double s0 = 0.0, s1 = 0.0;
         for (int i = rg; i < m; i += 8) {
@@ -355,34 +383,37 @@ __device__ double householder_qrcp2(double* X, int ld, int m, int n, double* wv,
         double part = (has_col && rg == 0) ? myn : 0.0;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
-        if (lane == 0) wv[16 + warp] = part;
+        if (lane == 0) wsum[warp] = part;
     }
-    auto warp_argmax = [&](int buf) {
-        double bv = active ? myn : -1.0;
-        int bi = cq;
-#pragma unroll
-        for (int o = 4; o < 32; o <<= 1) {
-            const double ov = __shfl_xor_sync(0xffffffffu, bv, o);
-            const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
-            if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
-        }
-        if (lane == 0) { wv[buf * 8 + warp] = bv; wi[buf * 8 + warp] = bi; }
+    // Pivot search: a non-negative double orders like its 64-bit pattern, so the warp's largest remaining
+    // norm comes from two redux.sync.max (high word, then low word among the lanes that tie on the high
+    // word) and a redux.sync.min on the column index among exact ties; lane 0 publishes (pattern, column).
+    // After the barrier every thread scans the <= 8 published pairs: exact argmax, smallest column on ties.
+    auto publish = [&](int buf) {
+        const unsigned hi = active ? (unsigned)__double2hiint(myn) + 1u : 0u;     // +1: an active zero column beats an inactive one
+        const unsigned lo = (unsigned)__double2loint(myn);
+        const unsigned mh = __reduce_max_sync(0xffffffffu, hi);
+        const unsigned ml = __reduce_max_sync(0xffffffffu, hi == mh ? lo : 0u);
+        const unsigned mc = __reduce_min_sync(0xffffffffu, (hi == mh && lo == ml) ? (unsigned)cq : 0xffffu);
+        if (lane == 0) { wk[buf * 24 + warp] = mh; wk[buf * 24 + 8 + warp] = ml; wk[buf * 24 + 16 + warp] = mc; }
     };
-    warp_argmax(0);
+    publish(0);
     __syncthreads();
     double fro2 = 0.0;
-    for (int w = 0; w < nw; ++w) fro2 += wv[16 + w];
+    for (int w = 0; w < nw; ++w) fro2 += wsum[w];
     const double thr2 = fro2 * 1e-30;
     int my_pstep = kk;
     double pend_beta = 0.0;
     int j = 0;
     for (; j < kk; ++j) {
         const int buf = j & 1;
-        double best = wv[buf * 8]; int bi = wi[buf * 8];
+        unsigned mh = wk[buf * 24], ml = wk[buf * 24 + 8], mc = wk[buf * 24 + 16];
         for (int w = 1; w < nw; ++w) {
-            const double ov = wv[buf * 8 + w]; const int oi = wi[buf * 8 + w];
-            if (ov > best || (ov == best && oi < bi)) { best = ov; bi = oi; }
+            const unsigned h2 = wk[buf * 24 + w], l2 = wk[buf * 24 + 8 + w], c2 = wk[buf * 24 + 16 + w];
+            if (h2 > mh || (h2 == mh && (l2 > ml || (l2 == ml && c2 < mc)))) { mh = h2; ml = l2; mc = c2; }
         }
+        const int bi = mh != 0u ? (int)mc : 0;
+        const double best = mh != 0u ? __hiloint2double((int)(mh - 1u), (int)ml) : 0.0;
         if ((j & 1) == 0 && !(best * (double)(n - j) > thr2)) break;
         const double* pc = X + (size_t)bi * ld;
         double bet, tau, scale;
@@ -430,7 +461,7 @@ __device__ double householder_qrcp2(double* X, int ld, int m, int n, double* wv,
             my_pstep = j;
             active = false;
         }
-        warp_argmax(buf ^ 1);
+        publish(buf ^ 1);
         __syncthreads();
         if (my_pstep == j && has_col && rg == 0) col[j] = pend_beta;
     }
@@ -501,8 +532,8 @@ __device__ int jacobi_rows2(double* M, int ld, int n, int nc, double fro2, doubl
                     const double dd = b - a;
                     const double g24 = 4.0 * g2;
                     const double h2 = fma(dd, dd, g24);
-                    const double u = fabs(dd) + h2 * rsqrt(h2);
-                    const double w = rsqrt(fma(u, u, g24));
+                    const double u = fabs(dd) + h2 * fast_rsqrt(h2);
+                    const double w = fast_rsqrt(fma(u, u, g24));
                     const double cs = u * w;
                     double sn = 2.0 * g * w;
                     if (dd < 0.0) sn = -sn;
