@@ -335,15 +335,20 @@ def main_ours(args):
         samp_flops = nb * model.sample_flops_per_chain_site(P) * n_dis * n_s * L * L
         samp_bytes = nb * model.sample_bytes_per_chain_site(P) * n_dis * n_s * L * L
         dominant = "build_rows_kernel" if phases["build"] >= phases["sample"] else "sample_rows_kernel"
+        traffic = None                                       # DRAM bytes per launch from the committed ncu capture (profiles/)
+        try:
+            traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(args.workload, {}).get(dominant)
+        except Exception:
+            pass
         if dominant == "build_rows_kernel":
             ach = build_flops / (build_ms * 1e-3) / 1e12
             roof = {"bound": "alu", "kernel": dominant, "achieved": ach, "peak": peak_dfma, "unit": "TFLOP/s", "frac": ach / peak_dfma,
-                    "traffic": None, "peak_source": "FP64 DFMA rate measured live by tnmc_fp64_peak_tflops(0) on this GPU",
+                    "traffic": traffic, "peak_source": "FP64 DFMA rate measured live by tnmc_fp64_peak_tflops(0) on this GPU",
                     "algorithmic_flops_per_launch_group": build_flops, "launches_per_group": nb}
         else:
             ach = samp_flops / (sample_ms * 1e-3) / 1e12
             roof = {"bound": "tensor", "kernel": dominant, "achieved": ach, "peak": peak_dmma, "unit": "TFLOP/s", "frac": ach / peak_dmma,
-                    "traffic": None, "peak_source": "FP64 DMMA (mma.sync.m8n8k4.f64) rate measured live by tnmc_fp64_peak_tflops(1)",
+                    "traffic": traffic, "peak_source": "FP64 DMMA (mma.sync.m8n8k4.f64) rate measured live by tnmc_fp64_peak_tflops(1)",
                     "algorithmic_flops_per_launch_group": samp_flops, "launches_per_group": nb}
         roof["other_kernels"] = {
             "sample_rows_kernel": {"ms": sample_ms, "tflops": samp_flops / (sample_ms * 1e-3) / 1e12, "frac_dmma_peak": samp_flops / (sample_ms * 1e-3) / 1e12 / peak_dmma,
