@@ -51,6 +51,10 @@ template <int P>
 struct BuildCfg {
     static constexpr int NT = 8 * P;          // threads per CTA: one quad per column of a 2P-column matrix
     static constexpr int D = 2 * P;           // doubled bond
+#ifndef TNMC_LPP
+#define TNMC_LPP 8
+#endif
+    static constexpr int LPP = TNMC_LPP;      // lanes per row pair in the Jacobi
     static constexpr int LDX = D + 4;         // column-major leading dim (= 4 mod 16: a half-warp of 4 quads hits 16 distinct 8-byte banks)
     static constexpr int LDM = D + 2;         // row length of the Jacobi operand (row-major)
     static constexpr int LDV = D + 1;         // row length of the selected right singular vectors
@@ -267,7 +271,7 @@ __global__ void __launch_bounds__(BuildCfg<P>::NT, BuildCfg<P>::CTAS_PER_SM) bui
             __syncthreads();
             const double thr2 = fro2 * 1e-30;      // sigma <= 1e-15 |M|_F: below the numerical rank
             PROF(4);
-            const int nsw = nrow >= 2 ? jacobi_rows2<(D + 15) / 16>(sMj, LDM, nrow, nc, fro2, thr2, args.flags) : 0;
+            const int nsw = nrow >= 2 ? jacobi_rows2<(D + 2 * Cfg::LPP - 1) / (2 * Cfg::LPP), Cfg::LPP>(sMj, LDM, nrow, nc, fro2, thr2, args.flags) : 0;
             PROF(5);
             PROF_ADD(8, nsw); PROF_ADD(9, 1);
             (void)nsw;

@@ -1,9 +1,11 @@
-// tnmc_linalg.cuh -- shared-memory dense kernels of the compression step (a-4, a-5):
-// Householder QR (+ explicit Q) and one-sided Jacobi SVD, written for one 256-thread CTA working
-// on one matrix of at most 128 x 64 doubles.  Everything here is latency-bound small linear
-// algebra; the design rule is: one block barrier per serial step, every trailing column (or every
-// row pair) handled in parallel by a group of lanes, scalar square roots and divisions kept off
-// the critical path.
+// tnmc_linalg.cuh -- shared-memory dense kernels of the compression step (a-4, a-5): Householder QR,
+// application of Q from its reflectors, Householder QR with column pivoting and one-sided Jacobi SVD,
+// for matrices of at most 64 x 64 doubles.  Everything here is a chain of small dependent steps; the
+// design rule is: at most one barrier per serial step, every trailing column handled by a quad of lanes
+// (every row pair by a group of lanes) with its loads batched in registers, square roots and divisions
+// replaced by MUFU-seeded rsqrt / reciprocal and kept off the critical path where possible.
+// (A one-lane-per-column, one-warp variant without any block barrier was measured and is slower: its
+// loops wait on shared-memory latency, profiles/r1e notes.)
 #pragma once
 #include "tnmc_common.cuh"
 
@@ -110,85 +112,6 @@ __device__ __forceinline__ void reflector_from_norm(double alpha, double nrm2, d
     }
 }
 
-// Householder QR of the m x n column-major matrix X (leading dim ld, odd) in shared memory,
-// m <= 4 * MAXK, n <= 8 * (warps per CTA).  On return the upper trapezoid holds R, the reflector
-// vectors (unit diagonal implied) sit below the diagonal, tau[j] their scalars; kk = min(m,n).
-// Step j: every trailing column is updated at once by a quad of lanes; the quad that owns column
-// j+1 goes on to build reflector j+1 from the freshly updated column (its remaining norm comes
-// out of the update for free), so a step costs one barrier.
-template <int MAXK>
-__device__ void householder_qr(double* X, int ld, int m, int n, double* tau) {
-    const int kk = m < n ? m : n;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int cs = lane >> 2, rg = lane & 3;
-    const unsigned qmask = 0xfu << (lane & ~3);
-    const int colidx = warp * 8 + cs;
-    if (warp == 0) {     // reflector 0
-        double ss = 0.0;
-        for (int i = lane; i < m; i += 32) { const double v = X[i]; ss = fma(v, v, ss); }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
-        double bet, t, scale;
-        reflector_from_norm(X[0], ss, bet, t, scale);
-        __syncwarp();
-        for (int i = 1 + lane; i < m; i += 32) X[i] *= scale;
-        if (lane == 0) { X[0] = bet; tau[0] = t; }
-    }
-    __syncthreads();
-    for (int j = 0; j < kk; ++j) {
-        const double* colj = X + (size_t)j * ld;
-        const double t = tau[j];
-        const int jj = j + 1 + colidx;
-        if (jj < n) {
-            double* col = X + (size_t)jj * ld;
-            double below2;
-            const double w = quad_dot_update<MAXK>(colj, col, j + 1, m, rg, qmask, t, col[j], below2);
-            if (rg == 0) col[j] -= w;
-            if (colidx == 0 && j + 1 < kk) {       // build reflector j+1 from the updated column
-                below2 += __shfl_xor_sync(qmask, below2, 1);
-                below2 += __shfl_xor_sync(qmask, below2, 2);
-                __syncwarp(qmask);
-                double bet, t1, scale;
-                reflector_from_norm(col[j + 1], below2, bet, t1, scale);
-                __syncwarp(qmask);
-                for (int i = j + 2 + rg; i < m; i += 4) col[i] *= scale;
-                if (rg == 0) { col[j + 1] = bet; tau[j + 1] = t1; }
-            }
-        }
-        __syncthreads();
-    }
-}
-
-// Overwrite the reflectors with the explicit thin Q (m x kk), in place (LAPACK dorg2r order).
-template <int MAXK>
-__device__ void householder_form_q(double* X, int ld, int m, int kk, const double* tau) {
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int cs = lane >> 2, rg = lane & 3;
-    const unsigned qmask = 0xfu << (lane & ~3);
-    const int colidx = warp * 8 + cs;
-    for (int j = kk - 1; j >= 0; --j) {
-        double* colj = X + (size_t)j * ld;
-        const double t = tau[j];
-        const int jj = j + 1 + colidx;
-        if (jj < kk) {
-            double* col = X + (size_t)jj * ld;
-            double below2;
-            // Q[j][jj] is 0 before H_j is applied: head = 0, and the new Q[j][jj] is -w
-            const double w = quad_dot_update<MAXK>(colj, col, j + 1, m, rg, qmask, t, 0.0, below2);
-            if (rg == 0) col[j] = -w;
-        }
-        __syncthreads();
-        for (int i = threadIdx.x; i < m; i += blockDim.x) {
-            double v;
-            if (i < j) v = 0.0;
-            else if (i == j) v = 1.0 - t;
-            else v = -t * colj[i];
-            colj[i] = v;
-        }
-        __syncthreads();
-    }
-}
-
 // ---------------------------------------------------------------------------------------------
 // Group versions: the CTA is split into thread groups (multiples of a warp) that each factor their
 // own matrix and synchronise on their own named barrier, so two factorizations of one site run
@@ -264,79 +187,6 @@ __device__ void householder_apply_g(const double* V, int ldv, const double* tau,
         }
     }
     (void)gn; (void)bar;
-}
-
-// Householder QR with column pivoting, R only:  X P = Q R  for the m x n column-major X in shared
-// memory (m <= 4 * MAXK, n <= 8 * warps).  On return the upper trapezoid of X holds R (kk = min(m,n)
-// rows), perm[j] the original index of column j.  cn (>= n doubles) is scratch.  Returns
-// sum of squares of X (= |X|_F^2) to all threads.
-// The pivot of step j is the column of largest REMAINING norm; those norms are not downdated but
-// summed afresh inside every trailing update, so they are exact.  Warp 0 picks the pivot, swaps it
-// into place and builds the reflector while the other warps wait: two barriers per step.
-// The point of the pivoting is what it does to the Jacobi SVD that follows ("SVD"):
-// the rows of R are graded and nearly orthogonal, and the sweeps drop from ~12 to ~5.
-template <int MAXK>
-__device__ double householder_qrcp(double* X, int ld, int m, int n, double* cn, int* perm, double* tau, int* ipiv) {
-    const int kk = m < n ? m : n;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int cs = lane >> 2, rg = lane & 3;
-    const unsigned qmask = 0xfu << (lane & ~3);
-    const int colidx = warp * 8 + cs;
-    if (colidx < n) {
-        const double* col = X + (size_t)colidx * ld;
-        double s0 = 0.0, s1 = 0.0;
-        for (int i = rg; i < m; i += 8) {
-            const double a = col[i]; s0 = fma(a, a, s0);
-            if (i + 4 < m) { const double b = col[i + 4]; s1 = fma(b, b, s1); }
-        }
-        double ss = s0 + s1;
-        ss += __shfl_xor_sync(qmask, ss, 1);
-        ss += __shfl_xor_sync(qmask, ss, 2);
-        if (rg == 0) { cn[colidx] = ss; perm[colidx] = colidx; }
-    }
-    __syncthreads();
-    double fro2 = 0.0;
-    for (int jj = 0; jj < n; ++jj) fro2 += cn[jj];
-    for (int j = 0; j < kk; ++j) {
-        if (warp == 0) {
-            // pivot: argmax of the remaining norms over columns j..n-1 (smallest index on ties)
-            double best = -1.0; int bi = j;
-            for (int jj = j + lane; jj < n; jj += 32) { const double v = cn[jj]; if (v > best) { best = v; bi = jj; } }
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                const double ov = __shfl_xor_sync(0xffffffffu, best, o);
-                const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
-                if (ov > best || (ov == best && oi < bi)) { best = ov; bi = oi; }
-            }
-            double* cj = X + (size_t)j * ld;
-            double* cp = X + (size_t)bi * ld;
-            if (bi != j) {
-                for (int i = lane; i < m; i += 32) { const double a = cj[i]; cj[i] = cp[i]; cp[i] = a; }
-                if (lane == 0) { cn[bi] = cn[j]; const int t = perm[j]; perm[j] = perm[bi]; perm[bi] = t; }
-            }
-            __syncwarp();
-            double bet, t, scale;
-            reflector_from_norm(cj[j], best, bet, t, scale);
-            __syncwarp();
-            for (int i = j + 1 + lane; i < m; i += 32) cj[i] *= scale;
-            if (lane == 0) { cj[j] = bet; tau[j] = t; }
-        }
-        __syncthreads();
-        const double* colj = X + (size_t)j * ld;
-        const double t = tau[j];
-        const int jj = j + 1 + colidx;
-        if (jj < n) {
-            double* col = X + (size_t)jj * ld;
-            double below2;
-            const double w = quad_dot_update<MAXK>(colj, col, j + 1, m, rg, qmask, t, col[j], below2);
-            below2 += __shfl_xor_sync(qmask, below2, 1);
-            below2 += __shfl_xor_sync(qmask, below2, 2);
-            if (rg == 0) { col[j] -= w; cn[jj] = below2; }
-        }
-        __syncthreads();
-    }
-    (void)ipiv;
-    return fro2;
 }
 
 // Householder QR with column pivoting, R only, second version: one barrier per step, no column swaps.
@@ -477,17 +327,17 @@ __device__ double householder_qrcp2(double* X, int ld, int m, int n, double* cn,
 // updated after a rotation and nothing is refreshed per sweep; and the rotation comes from two FP64
 // rsqrt with no division and no FP32 detour:
 //   d = b - a, h = sqrt(d^2 + 4 g^2), u = |d| + h, w = 1 / sqrt(u^2 + 4 g^2), cos = u w, sin = sign(d) 2 g w.
-// All n rows take part (n even); rows at or below thr2 are left alone.  NK = ceil(max nc / 16)
-// column pairs per lane.  Returns the sweeps done.
-template <int NK>
+// All n rows take part (n even); rows at or below thr2 are left alone.  LPP lanes per row pair (a power of
+// two <= 8), NK = ceil(max nc / (2 LPP)) column pairs per lane.  Returns the sweeps done.
+template <int NK, int LPP>
 __device__ int jacobi_rows2(double* M, int ld, int n, int nc, double fro2, double thr2, unsigned long long* flags) {
-    const int grp = threadIdx.x >> 3, t8 = threadIdx.x & 7;
+    const int grp = threadIdx.x / LPP, t8 = threadIdx.x % LPP;
     const int npairs = n >> 1;
-    const unsigned gmask = 0xffu << ((threadIdx.x & 31) & ~7);
+    const unsigned gmask = ((1u << LPP) - 1u) << ((threadIdx.x & 31) & ~(LPP - 1));
     const double rot2 = 256.0 * 4.930380657631324e-32;             // (16 eps)^2
     const double big2 = 1e-16;                                     // (1e-8)^2
     const double floor2 = 65536.0 * 4.930380657631324e-32 * fro2;  // (256 eps |M|_F)^2
-    const int c0 = 2 * t8;                                         // this lane's columns: c0 + 16 k, c0 + 16 k + 1
+    const int c0 = 2 * t8;                                         // this lane's columns: c0 + 2 LPP k, c0 + 2 LPP k + 1
     int sweep = 0;
     for (; sweep < 60; ++sweep) {
         int big = 0;
@@ -505,7 +355,7 @@ __device__ int jacobi_rows2(double* M, int ld, int n, int nc, double fro2, doubl
                 double2 xv[NK], yv[NK];
 #pragma unroll
                 for (int k = 0; k < NK; ++k) {
-                    const int c = c0 + 16 * k;
+                    const int c = c0 + 2 * LPP * k;
                     if (c < nc) {
                         xv[k] = *reinterpret_cast<const double2*>(x + c);
                         yv[k] = *reinterpret_cast<const double2*>(y + c);
@@ -520,7 +370,7 @@ __device__ int jacobi_rows2(double* M, int ld, int n, int nc, double fro2, doubl
                 }
                 a += a1; b += b1; g += g1;
 #pragma unroll
-                for (int o = 4; o > 0; o >>= 1) {
+                for (int o = LPP / 2; o > 0; o >>= 1) {
                     a += __shfl_xor_sync(gmask, a, o);
                     b += __shfl_xor_sync(gmask, b, o);
                     g += __shfl_xor_sync(gmask, g, o);
@@ -539,7 +389,7 @@ __device__ int jacobi_rows2(double* M, int ld, int n, int nc, double fro2, doubl
                     if (dd < 0.0) sn = -sn;
 #pragma unroll
                     for (int k = 0; k < NK; ++k) {
-                        const int c = c0 + 16 * k;
+                        const int c = c0 + 2 * LPP * k;
                         if (c < nc) {
                             double2 xn, yn;
                             xn.x = fma(cs, xv[k].x, -sn * yv[k].x);  yn.x = fma(sn, xv[k].x, cs * yv[k].x);
@@ -554,185 +404,6 @@ __device__ int jacobi_rows2(double* M, int ld, int n, int nc, double fro2, doubl
         }
         if (!__syncthreads_or(big)) { ++sweep; break; }
     }
-    if (sweep >= 60 && threadIdx.x == 0) raise_flag(flags, FLAG_JACOBI_LIMIT);
-    return sweep;
-}
-
-// One-sided (Hestenes) Jacobi on the ROWS of the n x nc row-major matrix M (row length ld, a
-// multiple of 2; nc <= 64): plane rotations from the left until all rows are mutually orthogonal,
-// so that row x ends as sigma_x * v_x^T (M = U Sigma V^T).  n must be even.
-//   * Eight lanes own one row pair of the round-robin (circle) schedule; each lane keeps its 8
-//     columns of both rows in registers between the dot product and the rotation.
-//   * Squared row norms are cached in `nrm2` (shared, >= n doubles), refreshed once per sweep and
-//     updated by the exact 2x2 congruence after every rotation, so a round needs one dot product.
-//   * The rotation angle only steers convergence, so tan(theta) is computed in FP32 from
-//     operands scaled by the pair's larger norm; cos is then refined in FP64 (two Newton steps of
-//     rsqrt) and sin = cos * tan, which keeps every rotation orthogonal to rounding error.
-//   * A pair is rotated whenever its cosine exceeds 16 eps (relative criterion: small rows are
-//     resolved as well as rounding allows -- the exact-chi parity cases need that).
-//   * Sweeps stop after the first one in which no pair was "unsettled".  A pair is unsettled when
-//     its cosine exceeds 1e-8 (then the float-accurate rotation just applied still leaves more
-//     than rounding level) AND |x.y| exceeds 256 eps |M|_F max(|x|,|y|): a row far smaller than
-//     |M|_F picks up eps |M|_F of rounding noise from every rotation with a large row, so its
-//     cosines against other small rows cannot settle below that floor however many sweeps are
-//     spent (measured: without the floor term, 14 sweeps on average instead of 9).
-//   * Rows whose squared norm is <= thr2 (numerically zero against |M|_F) are left alone.
-// Returns the number of sweeps done (all threads).
-__device__ int jacobi_rows(double* M, int ld, int n, int nc, double fro2, double thr2, double* nrm2,
-                           unsigned long long* flags) {
-    const int grp = threadIdx.x >> 3, t8 = threadIdx.x & 7;
-    const int ngrp = blockDim.x >> 3;
-    const int npairs = n >> 1;
-    const unsigned gmask = 0xffu << ((threadIdx.x & 31) & ~7);
-#ifdef JAC_ROT1
-    const double rot2 = 4.930380657631324e-32;
-#else
-    const double rot2 = 256.0 * 4.930380657631324e-32;            // (16 eps)^2
-#endif
-    const double big2 = 1e-16;                                    // (1e-8)^2
-#ifdef JAC_NOFLOOR
-    const double floor2 = 0.0;
-#else
-    const double floor2 = 65536.0 * 4.930380657631324e-32 * fro2;  // (256 eps |M|_F)^2
-#endif
-    const int c0 = 2 * t8;                         // this lane's columns: c0 + 16 k, c0 + 16 k + 1
-#ifdef TNMC_PROFILE
-    long long jacc[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
-    long long ts0 = clock64();
-#endif
-    int sweep = 0;
-    for (; sweep < 60; ++sweep) {
-        // refresh the cached norms
-        for (int x = grp; x < n; x += ngrp) {
-            double a = 0.0;
-            for (int c = c0; c < nc; c += 16) {
-                const double2 v = *reinterpret_cast<const double2*>(M + (size_t)x * ld + c);
-                a = fma(v.x, v.x, a); a = fma(v.y, v.y, a);
-            }
-#pragma unroll
-            for (int o = 4; o > 0; o >>= 1) a += __shfl_xor_sync(gmask, a, o);
-            if (t8 == 0) nrm2[x] = a;
-        }
-        __syncthreads();
-#ifdef TNMC_PROFILE
-        { const long long t_ = clock64(); jacc[5] += t_ - ts0; ts0 = t_; }
-#endif
-        int big = 0;
-        for (int round = 0; round < n - 1; ++round) {
-            for (int p = grp; p < npairs; p += ngrp) {
-                int r1, r2;
-                if (p == 0) { r1 = n - 1; r2 = round; }
-                else {
-                    r1 = round + p; if (r1 >= n - 1) r1 -= n - 1;
-                    r2 = round - p; if (r2 < 0) r2 += n - 1;
-                }
-                if (r1 > r2) { const int t = r1; r1 = r2; r2 = t; }
-#ifdef TNMC_PROFILE
-                long long tj0 = clock64();
-#define JPROF(slot) do { const long long t_ = clock64(); jacc[slot - 10] += t_ - tj0; tj0 = t_; } while (0)
-#else
-#define JPROF(slot)
-#endif
-                const double a = nrm2[r1], b = nrm2[r2];
-                if (!(a > thr2 && b > thr2)) continue;
-                double* x = M + (size_t)r1 * ld;
-                double* y = M + (size_t)r2 * ld;
-                double2 xv[4], yv[4];
-                double gp[4] = {0.0, 0.0, 0.0, 0.0};
-#pragma unroll
-                for (int k = 0; k < 4; ++k) {
-                    const int c = c0 + 16 * k;
-                    if (c < nc) {
-                        xv[k] = *reinterpret_cast<const double2*>(x + c);
-                        yv[k] = *reinterpret_cast<const double2*>(y + c);
-                    }
-                }
-#pragma unroll
-                for (int k = 0; k < 4; ++k)
-                    if (c0 + 16 * k < nc) gp[k] = fma(xv[k].y, yv[k].y, xv[k].x * yv[k].x);
-                double g = (gp[0] + gp[1]) + (gp[2] + gp[3]);
-#pragma unroll
-                for (int o = 4; o > 0; o >>= 1) g += __shfl_xor_sync(gmask, g, o);
-                const double mx = a > b ? a : b, ab = a * b, g2 = g * g;
-                JPROF(10);
-#ifdef TNMC_PROFILE
-                jacc[8] += 1;
-#endif
-                if (g2 > rot2 * ab) {
-                    big |= (g2 > big2 * ab) && (g2 > floor2 * mx);
-                    // tan(theta) = sign(d) 2g / (|d| + sqrt(d^2 + 4 g^2)),  d = b - a, in FP32 on scaled operands
-                    const double sc = __hiloint2double((2046 - ((__double2hiint(mx) >> 20) & 0x7ff)) << 20, 0);  // ~1/mx, a power of 2
-                    const float df = (float)((b - a) * sc), gf = (float)(g * sc);
-                    const float hf = sqrtf(fmaf(df, df, 4.0f * gf * gf));
-                    float tf = __fdividef(2.0f * gf, fabsf(df) + hf);
-                    if (df < 0.0f) tf = -tf;
-                    const double tt = (double)tf;
-                    const double x2 = fma(tt, tt, 1.0);
-                    double cs = (double)rsqrtf((float)x2);
-                    cs = cs * fma(-0.5 * x2, cs * cs, 1.5);
-                    cs = cs * fma(-0.5 * x2, cs * cs, 1.5);
-                    const double sn = cs * tt;
-                    JPROF(11);
-#ifdef TNMC_PROFILE
-                    jacc[9] += 1;
-#endif
-#pragma unroll
-                    for (int k = 0; k < 4; ++k) {
-                        const int c = c0 + 16 * k;
-                        if (c < nc) {
-                            double2 xn, yn;
-                            xn.x = fma(cs, xv[k].x, -sn * yv[k].x);  yn.x = fma(sn, xv[k].x, cs * yv[k].x);
-                            xn.y = fma(cs, xv[k].y, -sn * yv[k].y);  yn.y = fma(sn, xv[k].y, cs * yv[k].y);
-                            xv[k] = xn; yv[k] = yn;
-                            *reinterpret_cast<double2*>(x + c) = xn;
-                            *reinterpret_cast<double2*>(y + c) = yn;
-                        }
-                    }
-                    // new squared norms by the 2x2 congruence; where one of them came out of a
-                    // cancellation (a row was nearly annihilated) sum it directly
-                    const double cc = cs * cs, ss = sn * sn, csg = 2.0 * cs * sn * g;
-                    double na = cc * a - csg + ss * b;
-                    double nb = ss * a + csg + cc * b;
-                    if (na < 1e-4 * mx || nb < 1e-4 * mx) {
-                        double sx2 = 0.0, sy2 = 0.0;
-#pragma unroll
-                        for (int k = 0; k < 4; ++k)
-                            if (c0 + 16 * k < nc) {
-                                sx2 = fma(xv[k].x, xv[k].x, sx2); sx2 = fma(xv[k].y, xv[k].y, sx2);
-                                sy2 = fma(yv[k].x, yv[k].x, sy2); sy2 = fma(yv[k].y, yv[k].y, sy2);
-                            }
-#pragma unroll
-                        for (int o = 4; o > 0; o >>= 1) {
-                            sx2 += __shfl_xor_sync(gmask, sx2, o);
-                            sy2 += __shfl_xor_sync(gmask, sy2, o);
-                        }
-                        na = sx2; nb = sy2;
-                    }
-                    if (t8 == 0) { nrm2[r1] = na; nrm2[r2] = nb; }
-                    JPROF(12);
-                }
-            }
-#ifdef TNMC_PROFILE
-            long long tb0 = clock64();
-#endif
-            __syncthreads();
-#ifdef TNMC_PROFILE
-            jacc[3] += clock64() - tb0; jacc[4] += 1;
-#endif
-        }
-#ifdef TNMC_PROFILE
-        { const long long t_ = clock64(); jacc[6] += t_ - ts0; ts0 = t_; }
-#endif
-        const int more = __syncthreads_or(big);
-#ifdef TNMC_PROFILE
-        { const long long t_ = clock64(); jacc[7] += t_ - ts0; ts0 = t_; }
-#endif
-        if (!more) { ++sweep; break; }
-    }
-#ifdef TNMC_PROFILE
-    if (blockIdx.x == 0 && threadIdx.x == 0)
-        for (int i = 0; i < 10; ++i) atomicAdd(&g_build_prof[10 + i], (unsigned long long)jacc[i]);
-#endif
     if (sweep >= 60 && threadIdx.x == 0) raise_flag(flags, FLAG_JACOBI_LIMIT);
     return sweep;
 }
