@@ -66,7 +66,7 @@ __device__ __forceinline__ double quad_sum(double v) {
 }
 
 template <int P>
-__global__ void __launch_bounds__(SAMPLE_THREADS, 1) sample_rows_kernel(const SampleArgs args) {
+__global__ void __launch_bounds__(SAMPLE_THREADS, (P <= 16 ? 2 : 1)) sample_rows_kernel(const SampleArgs args) {
     constexpr int KT = P / 4;        // k tiles
     constexpr int NT = P / 4;        // n tiles (2P / 8)
     constexpr int JT = P / 8;        // 8-wide tiles per spin slice
