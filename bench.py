@@ -182,7 +182,7 @@ def main_reference(args):
 def main_ours(args):
     import torch
     import torch.distributed as dist
-    from paper_2509_19006_b200 import model, tnmc
+    from paper_2509_19006_b200 import model, shard, tnmc
 
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -199,7 +199,7 @@ def main_ours(args):
     P = model.pad_chi(chi)
     betas = list(c["betas"])
     # weak scaling: every rank owns its own n_dis disorders (global indices rank*n_dis ...); no collective on the data path
-    first = rank * n_dis
+    first = shard.first_disorder(rank, n_dis)
     Jr_np, Jd_np = make_couplings(L, n_dis, c["inst_seed"], first_disorder=first)
     Jr_h, Jd_h = torch.from_numpy(Jr_np).pin_memory(), torch.from_numpy(Jd_np).pin_memory()
     Jr, Jd = Jr_h.to(dev), Jd_h.to(dev)
@@ -279,12 +279,7 @@ def main_ours(args):
             tot_launch += launches
             for k in phases:
                 phases[k] += ph[k]
-    t = torch.tensor([tot_ms], dtype=torch.float64, device=dev)
-    a = torch.tensor([float(tot_acc)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(a, op=dist.ReduceOp.SUM)
-    ms_total, acc_total = t.item(), a.item()
+    ms_total, acc_total = shard.reduce_job(tot_ms, tot_acc, dev)
     value = acc_total / (ms_total * 1e-3)
 
     # ---- end to end: host buffers through tnmc_run_host, one host thread + stream per beta
@@ -310,14 +305,10 @@ def main_ours(args):
                 e_acc += sum(pool.map(host_pass, range(nb)))
             torch.cuda.synchronize()
             dt = time.perf_counter() - t0
-        te = torch.tensor([dt], dtype=torch.float64, device=dev)
-        ae = torch.tensor([float(e_acc)], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(te, op=dist.ReduceOp.MAX)
-            dist.all_reduce(ae, op=dist.ReduceOp.SUM)
+        dt_max, e_acc_sum = shard.reduce_job(dt, e_acc, dev)
         h2d = nb * (Jr_h.numel() + Jd_h.numel())
         d2h = sum(v.numel() * v.element_size() for o in outs for v in o.values() if v is not None)
-        e2e = {"value": ae.item() / te.item(), "unit": "samples/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h}
+        e2e = {"value": e_acc_sum / dt_max, "unit": "samples/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h}
 
     if rank == 0:
         # the nb launches of a phase run concurrently: duration of the group, algorithmic work of the group
