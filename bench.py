@@ -33,7 +33,9 @@ WORKLOADS = {
     "C3": ("C3", None, None, 0, "configs[2] 128x128 chi=32 256x256 FP64"),
     "C4s": ("C4", 148, 200, 23, "configs[3] 512x512 chi=32, slice of 148 disorders x 200 samples, checkpoint stride 23"),
     "C5s": ("C5", 74, 128, 32, "configs[4] 1024x1024 chi=32, slice of 74 disorders x 128 samples, checkpoint stride 32"),
+    "C5p": ("C5p", 500, 400, 32, "the paper headline setting (1024x1024, chi=8, PAPER.md:286) in FP64: slice of 500 disorders x 400 samples (one fifth of its 10^6 proposals), checkpoint stride 32"),
 }
+SLICES = ("C4s", "C5s", "C5p")      # steps of minutes: one warm-up step is enough to reach steady clocks (said in config.note)
 
 
 def parse():
@@ -43,6 +45,8 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="C2", choices=sorted(WORKLOADS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--prec", default="f64", choices=["f64", "f32"],
+                    help="f64: the parity path; f32: TNMC_F32_LOGSCALE (FP32 stack, TF32 tensor-core sampler, FP64 compression)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -203,8 +207,9 @@ def main_ours(args):
     Jr_np, Jd_np = make_couplings(L, n_dis, c["inst_seed"], first_disorder=first)
     Jr_h, Jd_h = torch.from_numpy(Jr_np).pin_memory(), torch.from_numpy(Jd_np).pin_memory()
     Jr, Jd = Jr_h.to(dev), Jd_h.to(dev)
-    need = tnmc.tnmc_workspace_bytes(L, chi, n_dis, n_s, ckpt_stride=ckpt)
-    need_h = tnmc.tnmc_run_host_workspace_bytes(L, chi, n_dis, n_s, ckpt_stride=ckpt)
+    prec = tnmc.TNMC_F32_LOGSCALE if args.prec == "f32" else tnmc.TNMC_F64
+    need = tnmc.tnmc_workspace_bytes(L, chi, n_dis, n_s, prec=prec, ckpt_stride=ckpt)
+    need_h = tnmc.tnmc_run_host_workspace_bytes(L, chi, n_dis, n_s, prec=prec, ckpt_stride=ckpt)
     W = tnmc.words(L)
     nb = len(betas)
     # the betas of a step are independent problems: each gets its own stream, workspace and outputs, and
@@ -226,7 +231,7 @@ def main_ours(args):
 
         def run(phase, i):
             if phase == "build":
-                ctxs[i] = tnmc.Context(L, chi, betas[i], Jr, Jd, n_s, first_disorder=first, ckpt_stride=ckpt, workspace=ws[i])
+                ctxs[i] = tnmc.Context(L, chi, betas[i], Jr, Jd, n_s, first_disorder=first, prec=prec, ckpt_stride=ckpt, workspace=ws[i])
                 ctxs[i].tnmc_build_envs(logZ[i])
             elif phase == "sample":
                 ctxs[i].tnmc_sample(n_s, c["seed"], cfg_bits=bits[i], logq=logq[i])
@@ -261,7 +266,8 @@ def main_ours(args):
         if world > 1:
             dist.barrier()
 
-    for _ in range(max(args.warmup, 3)):
+    n_warm = max(args.warmup, 1 if args.workload in SLICES else 3)
+    for _ in range(n_warm):
         step(False)
     phases = {"build": 0.0, "sample": 0.0, "energy": 0.0, "metropolis": 0.0}
     tot_ms, tot_acc, tot_launch = 0.0, 0, 0
@@ -292,11 +298,11 @@ def main_ours(args):
             torch.cuda.set_device(local_rank)
             with torch.cuda.stream(streams[i]):
                 outs[i] = tnmc.tnmc_run_host(L, chi, betas[i], Jr_h, Jd_h, n_s, c["seed"], ws[i], first_disorder=first,
-                                             ckpt_stride=ckpt, out=outs[i])
+                                             prec=prec, ckpt_stride=ckpt, out=outs[i])
             return int(outs[i]["n_accepted"].sum().item())
 
         with ThreadPoolExecutor(max_workers=nb) as pool:
-            for _ in range(2):
+            for _ in range(1 if args.workload in SLICES else 2):
                 list(pool.map(host_pass, range(nb)))
             e_acc = 0
             barrier()
@@ -324,7 +330,8 @@ def main_ours(args):
             pass
         hbm_peak = peaks.get("hbm_gbs", 6650.0)
         samp_flops = nb * model.sample_flops_per_chain_site(P) * n_dis * n_s * L * L
-        samp_bytes = nb * model.sample_bytes_per_chain_site(P) * n_dis * n_s * L * L
+        w_env = 4 if args.prec == "f32" else 8
+        samp_bytes = nb * model.sample_bytes_per_chain_site(P, w=w_env) * n_dis * n_s * L * L
         dominant = "build_rows_kernel" if phases["build"] >= phases["sample"] else "sample_rows_kernel"
         traffic = None                                       # DRAM bytes per launch from the committed ncu capture (profiles/)
         try:
@@ -354,8 +361,8 @@ def main_ours(args):
             cpu = {"value": acc_o / dt_o, "unit": "samples/s", "cores": threads_used(), "kind": "oracle", "seconds": dt_o,
                    "sample": f"{n_d} disorders x {n_so} samples x {len(betas)} betas of {args.workload} (whole path)"}
         line = {"metric": "accepted samples/s", "value": value, "unit": "samples/s", "n_gpus": world, "steps": args.steps,
-                "warmup": max(args.warmup, 3), "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak",
-                "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "warmup": n_warm, "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f64" if args.prec == "f64" else "f64 compression + tf32 sampling (fp32 stack)", "data": "synthetic",
                 "config": {"workload": args.workload, "note": c["note"], "L": L, "chi": chi, "betas": betas, "n_dis_per_gpu": n_dis,
                            "n_samples": n_s, "ckpt_stride": ckpt, "parallelism": f"dp{world} (disorders sharded, no collective)",
                            "l2": "flushed (256 MiB memset) between timed steps; env stack > L2",

@@ -69,7 +69,14 @@ typedef enum {
 } tnmc_status;
 
 typedef enum {
-    TNMC_F64 = 0 /* FP64 storage and arithmetic (the only precision in this round) */
+    TNMC_F64 = 0,          /* FP64 storage and arithmetic: the parity path (log Z 1e-10, conditionals 1e-9) */
+    TNMC_F32_LOGSCALE = 1  /* environment stack stored in FP32: every stored row has unit 2-norm and carries its
+                              log-scale separately (reading G7), so single precision has no range problem.
+                              Compression and sampling arithmetic stay FP64 on the FP32-rounded tensors.  Half
+                              the HBM footprint and traffic of the stack; conditionals agree with TNMC_F64 to
+                              ~1e-6, log Z to ~1e-7 relative (north_star reduced-precision tolerance: 1e-4);
+                              spins are not bit-identical to the FP64 path.  log q is the log of the
+                              probabilities actually used, so the Metropolis correction stays exact. */
 } tnmc_prec;
 
 /* indices into the array returned by tnmc_get_flags */

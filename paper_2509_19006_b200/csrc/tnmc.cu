@@ -31,8 +31,7 @@ static tnmc_status cuda_fail(tnmc_ctx* ctx, cudaError_t e, const char* what) {
 extern "C" size_t tnmc_workspace_bytes(int L, int chi, int n_dis, int n_samples_max, tnmc_prec prec,
                                        int ckpt_stride) {
     Plan p;
-    if (prec != TNMC_F64) return 0;
-    if (!make_plan(p, L, chi, n_dis, n_samples_max, ckpt_stride)) return 0;
+    if (!make_plan(p, L, chi, n_dis, n_samples_max, ckpt_stride, (int)prec)) return 0;
     return p.total;
 }
 
@@ -42,12 +41,12 @@ extern "C" tnmc_status tnmc_create(tnmc_ctx** out, int L, int chi, double beta, 
                                    void* workspace, size_t workspace_bytes, void* cuda_stream) {
     if (!out) return fail(nullptr, TNMC_EINVAL, "tnmc_create: out is NULL");
     *out = nullptr;
-    if (prec != TNMC_F64) return fail(nullptr, TNMC_EINVAL, "tnmc_create: only TNMC_F64 is implemented");
+    if (prec != TNMC_F64 && prec != TNMC_F32_LOGSCALE) return fail(nullptr, TNMC_EINVAL, "tnmc_create: unknown precision");
     if (!Jr || !Jd || !workspace) return fail(nullptr, TNMC_EINVAL, "tnmc_create: NULL pointer");
     if (!(beta >= 0.0) || !std::isfinite(beta)) return fail(nullptr, TNMC_EINVAL, "tnmc_create: beta must be finite and >= 0");
     if ((reinterpret_cast<uintptr_t>(workspace) & 255u) != 0) return fail(nullptr, TNMC_EINVAL, "tnmc_create: workspace must be 256-byte aligned");
     Plan p;
-    if (!make_plan(p, L, chi, n_dis, n_samples_max, ckpt_stride))
+    if (!make_plan(p, L, chi, n_dis, n_samples_max, ckpt_stride, (int)prec))
         return fail(nullptr, TNMC_EINVAL, "tnmc_create: need 2 <= L <= 4096, 2 <= chi <= 32, n_dis >= 1, n_samples_max >= 1, ckpt_stride >= 0");
     if (workspace_bytes < p.total) return fail(nullptr, TNMC_ENOMEM, "tnmc_create: workspace too small");
     int dev_count = 0;
@@ -111,7 +110,7 @@ static tnmc_status launch_build(tnmc_ctx* ctx, int m, int row_hi, int row_lo, in
     a.beta = ctx->beta; a.L = p.L; a.chi = p.chi; a.dis_begin = dis_begin;
     a.row_hi = row_hi; a.row_lo = row_lo;
     a.slot_of_row = ctx->map(m);
-    a.env = ctx->at<double>(p.off_env); a.env_dis_stride = p.env_dis_stride;
+    a.env = ctx->env(); a.env_dis_stride = p.env_dis_stride;
     a.qbuf = ctx->at<double>(p.off_qbuf);
     a.m0buf = ctx->at<double>(p.off_m0);
     a.logscale = ctx->at<double>(p.off_logscale);
@@ -125,8 +124,16 @@ static tnmc_status launch_build(tnmc_ctx* ctx, int m, int row_hi, int row_lo, in
     return TNMC_OK;
 }
 
-template <int P>
+template <int P, bool F32>
 static cudaError_t launch_sample_t(const tnmc_ctx* ctx, const SampleArgs& a, int tiles, int dis_count) {
+    if (F32) {
+        const int W32 = (a.L + 31) / 32;
+        const size_t smem32 = sizeof(float) * SAMPLE_STAGES * 2 * P * P + sizeof(uint32_t) * SAMPLE_CHAINS * W32;
+        cudaError_t e32 = cudaFuncSetAttribute(sample_rows_tf32_kernel<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem32);
+        if (e32 != cudaSuccess) return e32;
+        sample_rows_tf32_kernel<P><<<dim3(tiles, dis_count), SAMPLE_THREADS, smem32, ctx->stream>>>(a);
+        return cudaPeekAtLastError();
+    }
     const int W = (a.L + 31) / 32;
     const size_t smem = sizeof(double) * SAMPLE_STAGES * 2 * P * P + sizeof(uint32_t) * SAMPLE_CHAINS * W;
     cudaError_t e = cudaFuncSetAttribute(sample_rows_kernel<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -144,7 +151,7 @@ extern "C" tnmc_status tnmc_build_envs(tnmc_ctx* ctx, double* logZ) {
     const int* map0 = ctx->map(0);
     (void)map0;
     bottom_row_kernel<<<dim3(p.L, p.n_dis), 64, 0, ctx->stream>>>(
-        ctx->jview(), ctx->beta, p.L, p.P, ctx->at<double>(p.off_env), p.env_dis_stride,
+        ctx->jview(), ctx->beta, p.L, p.P, ctx->env(), p.env_dis_stride,
         p.perm_slot(p.L - 1), ctx->at<double>(p.off_logscale));
     CK_LAUNCH(ctx, "bottom_row_kernel");
     tnmc_status st = launch_build(ctx, 0, p.L - 1, 0, 0, p.n_dis);
@@ -152,7 +159,7 @@ extern "C" tnmc_status tnmc_build_envs(tnmc_ctx* ctx, double* logZ) {
     double* lz = logZ ? logZ : ctx->at<double>(p.off_logz);
     const int warps = 4;
     logz_kernel<<<(p.n_dis + warps - 1) / warps, warps * 32, 0, ctx->stream>>>(
-        p.L, p.chi, p.P, p.n_dis, ctx->at<double>(p.off_env), p.env_dis_stride, p.perm_slot(0),
+        p.L, p.chi, p.P, p.n_dis, ctx->env(), p.env_dis_stride, p.perm_slot(0),
         ctx->at<double>(p.off_logscale), lz, ctx->at<unsigned long long>(p.off_flags));
     CK_LAUNCH(ctx, "logz_kernel");
     ctx->built = true;
@@ -184,7 +191,7 @@ extern "C" tnmc_status tnmc_sample_ex(tnmc_ctx* ctx, int dis_begin, int dis_coun
     a.J = ctx->jview();
     a.beta = ctx->beta; a.L = p.L; a.chi = p.chi;
     a.dis_begin = dis_begin; a.n_samples = n_samples;
-    a.env = ctx->at<double>(p.off_env); a.env_dis_stride = p.env_dis_stride;
+    a.env = ctx->env(); a.env_dis_stride = p.env_dis_stride;
     a.renv = ctx->at<double>(p.off_renv);
     a.cfg_bits = cfg_bits; a.forced = forced_cfg_bits; a.logq = logq; a.probs = probs;
     a.seed_lo = (uint32_t)(seed & 0xffffffffu); a.seed_hi = (uint32_t)(seed >> 32);
@@ -202,9 +209,15 @@ extern "C" tnmc_status tnmc_sample_ex(tnmc_ctx* ctx, int dis_begin, int dis_coun
         } else { a.row_lo = 0; a.row_hi = p.L; }
         a.slot_of_row = ctx->map(m);
         cudaError_t e;
-        if (p.P == 8) e = launch_sample_t<8>(ctx, a, tiles, dis_count);
-        else if (p.P == 16) e = launch_sample_t<16>(ctx, a, tiles, dis_count);
-        else e = launch_sample_t<32>(ctx, a, tiles, dis_count);
+        if (p.f32) {
+            if (p.P == 8) e = launch_sample_t<8, true>(ctx, a, tiles, dis_count);
+            else if (p.P == 16) e = launch_sample_t<16, true>(ctx, a, tiles, dis_count);
+            else e = launch_sample_t<32, true>(ctx, a, tiles, dis_count);
+        } else {
+            if (p.P == 8) e = launch_sample_t<8, false>(ctx, a, tiles, dis_count);
+            else if (p.P == 16) e = launch_sample_t<16, false>(ctx, a, tiles, dis_count);
+            else e = launch_sample_t<32, false>(ctx, a, tiles, dis_count);
+        }
         if (e != cudaSuccess) return cuda_fail(ctx, e, "sample_rows_kernel");
         ctx->launches++;
     }
@@ -274,8 +287,8 @@ extern "C" tnmc_status tnmc_get_env_row(tnmc_ctx* ctx, int disorder, int row, do
     if (slot < 0) return fail(ctx, TNMC_ESTATE, "tnmc_get_env_row: row is not kept in checkpoint mode");
     // stage through the (currently idle) Q scratch of this disorder
     double* tmp = ctx->at<double>(p.off_qbuf) + (size_t)disorder * p.L * p.qsz;
-    const double* src = ctx->at<double>(p.off_env) + (size_t)disorder * p.env_dis_stride + (size_t)slot * p.L * p.tsz;
-    export_row_kernel<<<p.L, 128, 0, ctx->stream>>>(p.L, p.chi, p.P, src, tmp);
+    const size_t src = (size_t)disorder * p.env_dis_stride + (size_t)slot * p.L * p.tsz;
+    export_row_kernel<<<p.L, 128, 0, ctx->stream>>>(p.L, p.chi, p.P, ctx->env(), src, tmp);
     CK_LAUNCH(ctx, "export_row_kernel");
     CK(ctx, cudaMemcpyAsync(out, tmp, sizeof(double) * (size_t)p.L * p.chi * 2 * p.chi, cudaMemcpyDeviceToHost, ctx->stream));
     if (logscale_out)
@@ -293,9 +306,9 @@ struct HostPlan {
     size_t off_jr, off_jd, off_cfg, off_E, off_logq, off_acc, off_logz, off_cq, off_ce, off_ci, off_nacc,
            off_ctx, ctx_bytes, total;
 };
-bool make_host_plan(HostPlan& h, int L, int chi, int n_dis, int n_samples, int ckpt) {
+bool make_host_plan(HostPlan& h, int L, int chi, int n_dis, int n_samples, int ckpt, int prec) {
     Plan p;
-    if (!make_plan(p, L, chi, n_dis, n_samples, ckpt)) return false;
+    if (!make_plan(p, L, chi, n_dis, n_samples, ckpt, prec)) return false;
     const size_t nc = (size_t)n_dis * n_samples;
     size_t o = 0;
     h.off_jr = o;   o = align_up(o + (size_t)n_dis * L * L);
@@ -318,7 +331,7 @@ bool make_host_plan(HostPlan& h, int L, int chi, int n_dis, int n_samples, int c
 extern "C" size_t tnmc_run_host_workspace_bytes(int L, int chi, int n_dis, int n_samples, tnmc_prec prec,
                                                 int ckpt_stride) {
     HostPlan h;
-    if (prec != TNMC_F64 || !make_host_plan(h, L, chi, n_dis, n_samples, ckpt_stride)) return 0;
+    if (!make_host_plan(h, L, chi, n_dis, n_samples, ckpt_stride, (int)prec)) return 0;
     return h.total;
 }
 
@@ -329,7 +342,7 @@ extern "C" tnmc_status tnmc_run_host(int L, int chi, double beta, int n_dis, int
                                      uint32_t* out_cfg_bits, int32_t* out_E, double* out_logq,
                                      uint8_t* out_accepted, double* out_logZ, int64_t* out_n_accepted) {
     HostPlan h;
-    if (prec != TNMC_F64 || !make_host_plan(h, L, chi, n_dis, n_samples, ckpt_stride))
+    if (!make_host_plan(h, L, chi, n_dis, n_samples, ckpt_stride, (int)prec))
         return fail(nullptr, TNMC_EINVAL, "tnmc_run_host: bad sizes");
     if (!Jr_host || !Jd_host || !workspace) return fail(nullptr, TNMC_EINVAL, "tnmc_run_host: NULL pointer");
     if (workspace_bytes < h.total) return fail(nullptr, TNMC_ENOMEM, "tnmc_run_host: workspace too small");

@@ -39,8 +39,8 @@ struct BuildArgs {
     int dis_begin;               // CTA b works on disorder dis_begin + b
     int row_hi, row_lo;          // processes rows row_hi-1, ..., row_lo; row row_hi must be stored
     const int* slot_of_row;      // [L] device: env slot of each row for this pass (-1: not stored)
-    double* env;                 // env base
-    size_t env_dis_stride;       // doubles per disorder (n_slots * L * 2P^2)
+    EnvRef env;                  // env base (FP64 or FP32 storage)
+    size_t env_dis_stride;       // elements per disorder (n_slots * L * 2P^2)
     double* qbuf;                // scratch, per disorder L * QSZ doubles (reflectors of the QR sweep)
     double* m0buf;               // scratch, per disorder D*D doubles (M before rotation; used when P == 32)
     double* logscale;            // (n_dis, L): logscale of every row (written for rows built)
@@ -102,15 +102,16 @@ __global__ void __launch_bounds__(BuildCfg<P>::NT, BuildCfg<P>::CTAS_PER_SM) bui
     const int half = tid >= HALF ? 1 : 0, gt = tid - half * HALF;
     const int d = args.dis_begin + blockIdx.x;
     const int L = args.L, chi = args.chi;
+    const int f32 = args.env.f32;        // selects the fragment order of the stored tensors
     const double beta = args.beta;
-    double* env_d = args.env + (size_t)d * args.env_dis_stride;
+    const size_t env_d = (size_t)d * args.env_dis_stride;
     double* qbuf_d = args.qbuf + (size_t)d * (size_t)L * Cfg::QSZ;
     double* ls_d = args.logscale + (size_t)d * L;
 
     PROF_DECL
     for (int r = args.row_hi - 1; r >= args.row_lo; --r) {
-        const double* env_in = env_d + (size_t)args.slot_of_row[r + 1] * L * TSZ;
-        double* env_out = env_d + (size_t)args.slot_of_row[r] * L * TSZ;
+        const size_t env_in = env_d + (size_t)args.slot_of_row[r + 1] * L * TSZ;
+        const size_t env_out = env_d + (size_t)args.slot_of_row[r] * L * TSZ;
         double logs = 0.0;   // all threads carry the same value
 
         // ------------------------------------------------------------------ A. QR sweep, left -> right
@@ -120,15 +121,15 @@ __global__ void __launch_bounds__(BuildCfg<P>::NT, BuildCfg<P>::CTAS_PER_SM) bui
         for (int c = 0; c < L; ++c) {
             const int bl = row_bond(L, chi, r + 1, c), br = row_bond(L, chi, r + 1, c + 1);
             const int q = sq[c];
-            const double* Ain = env_in + (size_t)c * TSZ;
-            for (int t = tid; t < TSZ; t += NT) sA[t] = Ain[t];
+            const size_t Ain = env_in + (size_t)c * TSZ;
+            for (int t = tid; t < TSZ; t += NT) sA[t] = args.env.ld(Ain + t);
             __syncthreads();
             {   // C_a[i][k] = sum_m B_d[a][m] A[i][m][k]      (Eq. 7: B_d[a][m] = exp(beta Jd (2a-1)(2m-1)))
                 const int jd = args.J.jd(d, r, c);
                 const double w_same = exp(beta * jd), w_diff = exp(-beta * jd);
                 for (int t = tid; t < 2 * bl * br; t += NT) {
                     const int k = t % br, i = (t / br) % bl, a = t / (br * bl);
-                    sU[(a * P + i) * LDU + k] = w_same * sA[env_off(P, i, a, k)] + w_diff * sA[env_off(P, i, 1 - a, k)];
+                    sU[(a * P + i) * LDU + k] = w_same * sA[env_off_p(P, i, a, k, f32)] + w_diff * sA[env_off_p(P, i, 1 - a, k, f32)];
                 }
             }
             __syncthreads();
@@ -233,7 +234,7 @@ __global__ void __launch_bounds__(BuildCfg<P>::NT, BuildCfg<P>::CTAS_PER_SM) bui
                                           sX + (size_t)half * kprev * LDX, LDX, kprev, gt, HALF, 1 + half);
             }
             __syncthreads();
-            double* Aout = env_out + (size_t)c * TSZ;
+            const size_t Aout = env_out + (size_t)c * TSZ;
             if (c == 0) {
                 // P-C2 step 3: A_0 (1,2,k_1) = M (1 x nc); divide by its norm, add log to logscale
                 double ss = 0.0;
@@ -247,9 +248,9 @@ __global__ void __launch_bounds__(BuildCfg<P>::NT, BuildCfg<P>::CTAS_PER_SM) bui
                 __syncthreads();
                 for (int t = tid; t < TSZ; t += NT) stage[t] = 0.0;
                 __syncthreads();
-                if (tid < nc) stage[env_off(P, 0, tid / kprev, tid % kprev)] = m0;
+                if (tid < nc) stage[env_off_p(P, 0, tid / kprev, tid % kprev, f32)] = m0;
                 __syncthreads();
-                for (int t = tid; t < TSZ; t += NT) Aout[t] = stage[t];
+                for (int t = tid; t < TSZ; t += NT) args.env.st(Aout + t, stage[t]);
                 __syncthreads();
                 break;
             }
@@ -315,11 +316,11 @@ __global__ void __launch_bounds__(BuildCfg<P>::NT, BuildCfg<P>::CTAS_PER_SM) bui
                     // orthonormal completion); it is stored as a zero row
                     const double v = sx * sx > thr2 ? sMj[(size_t)x * LDM + col] / sx : 0.0;
                     sV[(size_t)yp * LDV + col] = v;     // col = (a, y) = a * kprev + y
-                    stage[env_off(P, yp, col / kprev, col % kprev)] = v;
+                    stage[env_off_p(P, yp, col / kprev, col % kprev, f32)] = v;
                 }
             }
             __syncthreads();
-            for (int t = tid; t < TSZ; t += NT) Aout[t] = stage[t];
+            for (int t = tid; t < TSZ; t += NT) args.env.st(Aout + t, stage[t]);
             // Pc_next[x][y'] = sum_col M[x][col] V_k[col][y']   (= M V_k, projector form of P-C2 step 2)
             for (int t = tid; t < q * k; t += NT) {
                 const int x = t % q, yp = t / q;
@@ -346,20 +347,20 @@ __global__ void __launch_bounds__(BuildCfg<P>::NT, BuildCfg<P>::CTAS_PER_SM) bui
 //   A_0[0][a][b] = B(Jr[L-1][0])[a][b];  A_c[l][a][b] = delta(l,a) B(Jr[L-1][c])[a][b];
 //   A_{L-1}[l][a][0] = delta(l,a).   One CTA per (site, disorder).
 // ---------------------------------------------------------------------------------------------
-__global__ void bottom_row_kernel(JView J, double beta, int L, int P, double* env, size_t env_dis_stride,
+__global__ void bottom_row_kernel(JView J, double beta, int L, int P, EnvRef env, size_t env_dis_stride,
                                   int slot, double* logscale) {
     const int c = blockIdx.x, d = blockIdx.y;
     const int TSZ = 2 * P * P;
-    double* A = env + (size_t)d * env_dis_stride + ((size_t)slot * L + c) * TSZ;
-    for (int t = threadIdx.x; t < TSZ; t += blockDim.x) A[t] = 0.0;
+    const size_t A = (size_t)d * env_dis_stride + ((size_t)slot * L + c) * TSZ;
+    for (int t = threadIdx.x; t < TSZ; t += blockDim.x) env.st(A + t, 0.0);
     __syncthreads();
     if (threadIdx.x < 8) {
         const int l = threadIdx.x >> 2, a = (threadIdx.x >> 1) & 1, b = threadIdx.x & 1;
         const int jr = (c == L - 1) ? 0 : J.jr(d, L - 1, c);
         const double bm = exp(beta * jr * (2 * a - 1) * (2 * b - 1));
-        if (c == 0) { if (l == 0) A[env_off(P, 0, a, b)] = bm; }
-        else if (c == L - 1) { if (b == 0 && l == a) A[env_off(P, l, a, 0)] = 1.0; }
-        else if (l == a) A[env_off(P, l, a, b)] = bm;
+        if (c == 0) { if (l == 0) env.st(A + env_off_p(P, 0, a, b, env.f32), bm); }
+        else if (c == L - 1) { if (b == 0 && l == a) env.st(A + env_off_p(P, l, a, 0, env.f32), 1.0); }
+        else if (l == a) env.st(A + env_off_p(P, l, a, b, env.f32), bm);
     }
     if (c == 0 && threadIdx.x == 0) logscale[(size_t)d * L + (L - 1)] = 0.0;
 }
@@ -369,22 +370,22 @@ __global__ void bottom_row_kernel(JView J, double beta, int L, int P, double* en
 // the sum taken as the product over c of sum_a A_c[:,a,:] with a running max-abs rescale.
 // One warp per disorder; lane j carries component j of the running row vector.
 // ---------------------------------------------------------------------------------------------
-__global__ void logz_kernel(int L, int chi, int P, int n_dis, const double* env, size_t env_dis_stride,
+__global__ void logz_kernel(int L, int chi, int P, int n_dis, EnvRef env, size_t env_dis_stride,
                             int slot0, const double* logscale, double* logZ, unsigned long long* flags) {
     const int d = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (d >= n_dis) return;
     const int lane = threadIdx.x & 31;
     const int TSZ = 2 * P * P;
-    const double* row = env + (size_t)d * env_dis_stride + (size_t)slot0 * L * TSZ;
+    const size_t row = (size_t)d * env_dis_stride + (size_t)slot0 * L * TSZ;
     double v = lane == 0 ? 1.0 : 0.0;   // component `lane` of the running vector (P <= 32)
     double lg = logscale[(size_t)d * L];
     for (int c = 0; c < L; ++c) {
-        const double* A = row + (size_t)c * TSZ;
+        const size_t A = row + (size_t)c * TSZ;
         const int bl = row_bond(L, chi, 0, c), br = row_bond(L, chi, 0, c + 1);
         double acc = 0.0;
         for (int i = 0; i < bl; ++i) {
             const double vi = __shfl_sync(0xffffffffu, v, i);
-            if (lane < br) acc += vi * (A[env_off(P, i, 0, lane)] + A[env_off(P, i, 1, lane)]);
+            if (lane < br) acc += vi * (env.ld(A + env_off_p(P, i, 0, lane, env.f32)) + env.ld(A + env_off_p(P, i, 1, lane, env.f32)));
         }
         double mx = fabs(acc);
 #pragma unroll
@@ -425,12 +426,12 @@ __global__ void pack_couplings_kernel(const int8_t* Jr, const int8_t* Jd, int n_
 }
 
 // Export one stored row in the paper's layout (L, chi, 2, chi) -- test/inspection hook.
-__global__ void export_row_kernel(int L, int chi, int P, const double* row, double* out) {
+__global__ void export_row_kernel(int L, int chi, int P, EnvRef env, size_t row, double* out) {
     const int c = blockIdx.x;
     const int TSZ = 2 * P * P;
     for (int t = threadIdx.x; t < chi * 2 * chi; t += blockDim.x) {
         const int j = t % chi, a = (t / chi) & 1, i = t / (2 * chi);
-        out[(size_t)c * chi * 2 * chi + t] = row[(size_t)c * TSZ + env_off(P, i, a, j)];
+        out[(size_t)c * chi * 2 * chi + t] = env.ld(row + (size_t)c * TSZ + env_off_p(P, i, a, j, env.f32));
     }
 }
 

@@ -40,6 +40,39 @@ __host__ __device__ __forceinline__ int env_off(int P, int i, int a, int j) {
     return ((kt * (P >> 2) + nt) * 32 + g * 4 + q);
 }
 
+// FP32 storage (TNMC_F32_LOGSCALE) uses the fragment order of mma.sync.m16n8k8.tf32 instead: k-tile kt
+// holds the eight left-bond indices i = 8*kt + 2*q + h (q = 0..3 <-> k-slots q and q+4 for h = 0, 1), the
+// two values of a lane are adjacent:  offset = ((kt * NT + nt) * 32 + g*4 + q) * 2 + h,  NT = P/4,
+// so a lane reads its (b0, b1) pair with one 8-byte load and, as in the FP64 layout, the accumulator
+// fragment of one site (columns 2q, 2q+1 of each n-tile) is the A fragment of the next.
+__host__ __device__ __forceinline__ int env_off32(int P, int i, int a, int j) {
+    const int kt = i >> 3;
+    const int q = (i & 7) >> 1, h = i & 1;
+    const int nt = a * (P >> 3) + (j >> 3);
+    const int g = j & 7;
+    return ((kt * (P >> 2) + nt) * 32 + g * 4 + q) * 2 + h;
+}
+__host__ __device__ __forceinline__ int env_off_p(int P, int i, int a, int j, int f32) {
+    return f32 ? env_off32(P, i, a, j) : env_off(P, i, a, j);
+}
+
+// The environment stack is stored in FP64 (TNMC_F64) or in FP32 (TNMC_F32_LOGSCALE: every stored row has
+// unit 2-norm and carries its log-scale separately, so single precision has no range problem); offsets are
+// in elements either way.
+struct EnvRef {
+    void* base;
+    int f32;
+    __device__ __forceinline__ double ld(size_t i) const {
+        return f32 ? (double)reinterpret_cast<const float*>(base)[i] : reinterpret_cast<const double*>(base)[i];
+    }
+    __device__ __forceinline__ void st(size_t i, double v) const {
+        if (f32) reinterpret_cast<float*>(base)[i] = (float)v; else reinterpret_cast<double*>(base)[i] = v;
+    }
+    __host__ __device__ __forceinline__ const char* bytes(size_t i) const {
+        return reinterpret_cast<const char*>(base) + i * (f32 ? 4 : 8);
+    }
+};
+
 // Bond dimension left of column c (c = 0..L) of the stored row r after compression (P-C2):
 // min(chi, 2^min(c, L-c), 2^(L-r)); 1 at the two ends.  Closed form of the recurrences
 //   q_{c+1} = min(2 q_c, D'_{c+1}),  k_c = min(chi, q_c, 2 k_{c+1})

@@ -10,6 +10,7 @@
 #include "tnmc_common.cuh"
 #include "tnmc_energy.cuh"
 #include "tnmc_sample.cuh"
+#include "tnmc_sample_tf32.cuh"
 
 namespace tnmc {
 
@@ -22,6 +23,7 @@ inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 //              the ping-pong pair of the first pass).  Segment j = rows [jk, min((j+1)k, L)).
 struct Plan {
     int L = 0, chi = 0, P = 0, W = 0, n_dis = 0, n_samples_max = 0, ckpt = 0;
+    int f32 = 0;                    // environment stack stored in FP32 (TNMC_F32_LOGSCALE)
     int n_seg = 1, n_slots = 0, n_seg_slots = 0, n_maps = 1, tiles = 1;
     size_t tsz = 0;                 // doubles per site tensor
     size_t env_dis_stride = 0;      // doubles per disorder
@@ -59,7 +61,9 @@ struct Plan {
     int seg_end(int j) const { const int h = (j + 1) * ckpt; return h < L ? h : L; }
 };
 
-inline bool make_plan(Plan& p, int L, int chi, int n_dis, int n_samples_max, int ckpt) {
+inline bool make_plan(Plan& p, int L, int chi, int n_dis, int n_samples_max, int ckpt, int prec = 0) {
+    if (prec != 0 && prec != 1) return false;
+    p.f32 = prec == 1;
     if (L < 2 || L > 4096 || chi < 2 || chi > 32 || n_dis < 1 || n_samples_max < 1 || ckpt < 0) return false;
     if (ckpt >= L) ckpt = 0;
     p.L = L; p.chi = chi; p.P = pad_chi(chi); p.W = (L + 31) / 32; p.n_dis = n_dis;
@@ -81,7 +85,7 @@ inline bool make_plan(Plan& p, int L, int chi, int n_dis, int n_samples_max, int
     p.off_flags = o;    o = align_up(o + sizeof(unsigned long long) * N_FLAGS);
     p.off_logscale = o; o = align_up(o + sizeof(double) * (size_t)n_dis * L);
     p.off_logz = o;     o = align_up(o + sizeof(double) * (size_t)n_dis);
-    p.off_env = o;      o = align_up(o + sizeof(double) * (size_t)n_dis * p.env_dis_stride);
+    p.off_env = o;      o = align_up(o + (p.f32 ? sizeof(float) : sizeof(double)) * (size_t)n_dis * p.env_dis_stride);
     p.off_qbuf = o;     o = align_up(o + sizeof(double) * (size_t)n_dis * L * p.qsz);
     p.off_m0 = o;       o = align_up(o + sizeof(double) * (size_t)n_dis * 4 * p.P * p.P);
     p.off_renv = o;     o = align_up(o + sizeof(double) * (size_t)n_dis * p.tiles * L * SAMPLE_CHAINS * p.P);
@@ -109,4 +113,5 @@ struct tnmc_ctx {
         return v;
     }
     const int* map(int m) const { return at<int>(plan.off_maps) + (size_t)m * plan.L; }
+    tnmc::EnvRef env() const { tnmc::EnvRef e; e.base = ws + plan.off_env; e.f32 = plan.f32; return e; }
 };

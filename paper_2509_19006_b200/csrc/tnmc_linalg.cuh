@@ -341,14 +341,14 @@ __device__ int jacobi_rows2(double* M, int ld, int n, int nc, double fro2, doubl
     int sweep = 0;
     for (; sweep < 60; ++sweep) {
         int big = 0;
+        // round-robin (circle) schedule: pair 0 is (n-1, round), pair p >= 1 is ((round + p) mod (n-1),
+        // (round - p) mod (n-1)); both members advance by one per round
+        int q1 = grp, q2 = grp == 0 ? 0 : n - 1 - grp;
         for (int round = 0; round < n - 1; ++round) {
             if (grp < npairs) {
-                int r1, r2;
-                if (grp == 0) { r1 = n - 1; r2 = round; }
-                else {
-                    r1 = round + grp; if (r1 >= n - 1) r1 -= n - 1;
-                    r2 = round - grp; if (r2 < 0) r2 += n - 1;
-                }
+                int r1 = grp == 0 ? n - 1 : q1, r2 = q2;
+                if (++q1 == n - 1) q1 = 0;
+                if (++q2 == n - 1) q2 = 0;
                 if (r1 > r2) { const int t = r1; r1 = r2; r2 = t; }
                 double* x = M + (size_t)r1 * ld;
                 double* y = M + (size_t)r2 * ld;

@@ -33,8 +33,8 @@ struct SampleArgs {
     int dis_begin, n_samples;
     int row_lo, row_hi;              // rows [row_lo, row_hi)
     const int* slot_of_row;          // [L] device
-    const double* env;
-    size_t env_dis_stride;
+    EnvRef env;                      // FP64 storage here; FP32 storage is read by tnmc_sample_tf32.cuh
+    size_t env_dis_stride;           // elements per disorder
     double* renv;                    // scratch: per CTA  L * SAMPLE_CHAINS * P doubles
     uint32_t* cfg_bits;              // (dis_count, n_samples, L, W)
     const uint32_t* forced;          // or nullptr
@@ -84,7 +84,7 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, (P <= 16 ? 2 : 1)) sample_rows
     const int tile = blockIdx.x;
     const double beta = args.beta;
     const double eb = exp(beta), emb = exp(-beta);
-    const double* env_d = args.env + (size_t)d * args.env_dis_stride;
+    const double* env_d = reinterpret_cast<const double*>(args.env.base) + (size_t)d * args.env_dis_stride;
     double* renv = args.renv + ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * (size_t)L * SAMPLE_CHAINS * P;
 
     // chain handled as M-tile mt, row g of this warp
