@@ -42,15 +42,19 @@ __host__ __device__ __forceinline__ int env_off(int P, int i, int a, int j) {
 
 // FP32 storage (TNMC_F32_LOGSCALE) uses the fragment order of mma.sync.m16n8k8.tf32 instead: k-tile kt
 // holds the eight left-bond indices i = 8*kt + 2*q + h (q = 0..3 <-> k-slots q and q+4 for h = 0, 1), the
-// two values of a lane are adjacent:  offset = ((kt * NT + nt) * 32 + g*4 + q) * 2 + h,  NT = P/4,
-// so a lane reads its (b0, b1) pair with one 8-byte load and, as in the FP64 layout, the accumulator
-// fragment of one site (columns 2q, 2q+1 of each n-tile) is the A fragment of the next.
+// two values of a lane are adjacent and the even columns g of a tile come before the odd ones:
+//   offset = ((kt * NT + nt) * 32 + (g&1)*16 + (g>>1)*4 + q) * 2 + h,  NT = P/4.
+// The left sweep (contraction over i) reads its (b0, b1) pair with one conflict-free 8-byte load; the
+// right sweep (contraction over j) reads the same tile transposed -- lane (g, q) needs
+// (i = 8 it + g, j = 8 kt + 2q + e) -- at words 8q + g (e = 0) and 32 + 8q + g (e = 1): conflict-free too,
+// which is what the even/odd split is for.  As in the FP64 layout the accumulator fragment of one site
+// (columns 2q, 2q+1 of each n-tile) is the A fragment of the next.
 __host__ __device__ __forceinline__ int env_off32(int P, int i, int a, int j) {
     const int kt = i >> 3;
     const int q = (i & 7) >> 1, h = i & 1;
     const int nt = a * (P >> 3) + (j >> 3);
     const int g = j & 7;
-    return ((kt * (P >> 2) + nt) * 32 + g * 4 + q) * 2 + h;
+    return ((kt * (P >> 2) + nt) * 32 + (g & 1) * 16 + (g >> 1) * 4 + q) * 2 + h;
 }
 __host__ __device__ __forceinline__ int env_off_p(int P, int i, int a, int j, int f32) {
     return f32 ? env_off32(P, i, a, j) : env_off(P, i, a, j);

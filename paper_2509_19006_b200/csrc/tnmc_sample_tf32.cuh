@@ -144,8 +144,8 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, 2) sample_rows_tf32_kernel(con
 #pragma unroll
                 for (int nt = 0; nt < NT; ++nt) {
                     const int a = nt / JT, it = nt % JT;
-                    const int off = (((it * NT + a * JT + kt) * 32 + (2 * q) * 4 + (g >> 1)) * 2) + (g & 1);   // env_off32(P, 8 it + g, a, 8 kt + 2q)
-                    const float b0 = T[off], b1 = T[off + 8];
+                    const int off = (it * NT + a * JT + kt) * 64 + 8 * q + g;   // env_off32(P, 8 it + g, a, 8 kt + 2q); the odd column is 32 words on
+                    const float b0 = T[off], b1 = T[off + 32];
                     mma16808_tf32(acc[0][nt][0], acc[0][nt][1], acc[1][nt][0], acc[1][nt][1],
                                   vf[0][2 * kt], vf[1][2 * kt], vf[0][2 * kt + 1], vf[1][2 * kt + 1], b0, b1);
                 }
@@ -223,7 +223,7 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, 2) sample_rows_tf32_kernel(con
             for (int kt = 0; kt < KT8; ++kt)
 #pragma unroll
                 for (int nt = 0; nt < NT; ++nt) {
-                    const float2 b = *(reinterpret_cast<const float2*>(T) + (kt * NT + nt) * 32 + lane);
+                    const float2 b = *(reinterpret_cast<const float2*>(T) + (kt * NT + nt) * 32 + (g & 1) * 16 + (g >> 1) * 4 + q);
                     mma16808_tf32(acc[0][nt][0], acc[0][nt][1], acc[1][nt][0], acc[1][nt][1],
                                   vf[0][2 * kt], vf[1][2 * kt], vf[0][2 * kt + 1], vf[1][2 * kt + 1], b.x, b.y);
                 }
