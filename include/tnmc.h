@@ -70,13 +70,18 @@ typedef enum {
 
 typedef enum {
     TNMC_F64 = 0,          /* FP64 storage and arithmetic: the parity path (log Z 1e-10, conditionals 1e-9) */
-    TNMC_F32_LOGSCALE = 1  /* environment stack stored in FP32: every stored row has unit 2-norm and carries its
-                              log-scale separately (reading G7), so single precision has no range problem.
-                              Compression and sampling arithmetic stay FP64 on the FP32-rounded tensors.  Half
-                              the HBM footprint and traffic of the stack; conditionals agree with TNMC_F64 to
-                              ~1e-6, log Z to ~1e-7 relative (north_star reduced-precision tolerance: 1e-4);
-                              spins are not bit-identical to the FP64 path.  log q is the log of the
-                              probabilities actually used, so the Metropolis correction stays exact. */
+    TNMC_F32_LOGSCALE = 1  /* reduced precision (BASELINE configs[2]; the paper's own dtype is torch.float):
+                              environment stack stored in FP32 -- every stored row has unit 2-norm and carries
+                              its log-scale separately (reading G7), so single precision has no range problem --
+                              and sampling contractions on TF32 tensor cores (mma.sync.m16n8k8, FP32 accumulate,
+                              environments normalised per site).  The compression stays FP64 (it has to resolve
+                              sigma_chi / sigma_1 ~ 1e-9).  Conditional probabilities, the draw and log q are
+                              evaluated in FP64 from the FP32 weights with p0 = 1 - p1: q is a normalised
+                              distribution and log q is the log of the probabilities actually used, so the
+                              Metropolis correction stays exact.  log Z agrees with TNMC_F64 to ~1e-7 relative
+                              (north_star reduced-precision tolerance 1e-4); conditionals carry ~1e-3 of TF32
+                              noise, spins are not bit-identical to the FP64 path, the acceptance is lower.
+                              TNMC_FLAG_RHO_ZERO is informational in this mode. */
 } tnmc_prec;
 
 /* indices into the array returned by tnmc_get_flags */
