@@ -120,21 +120,22 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, (P <= 16 ? 2 : 1)) sample_rows
     // ---- tensor stream: per row the right sweep consumes sites L-1..1, the left sweep sites 0..L-1
     const int steps_per_row = 2 * L - 1;
     const int n_rows = args.row_hi - args.row_lo;
-    const long long total_steps = (long long)n_rows * steps_per_row;
-    auto issue_prefetch = [&](long long s) {
-        if (s < total_steps) {
-            const int rr = args.row_lo + (int)(s / steps_per_row);
-            const int t = (int)(s % steps_per_row);
-            const int site = t < L - 1 ? (L - 1 - t) : (t - (L - 1));
-            const double* src = env_d + ((size_t)args.slot_of_row[rr] * L + site) * TSZ;
-            double* dst = sT + (size_t)(s % SAMPLE_STAGES) * TSZ;
+    (void)n_rows;
+    // the tensor stream is addressed with running counters (a 64-bit division per site costs ~60 instructions)
+    int pf_r = args.row_lo, pf_t = 0, pf_stage = 0, cur_stage = 0;
+    auto issue_prefetch = [&]() {
+        if (pf_r < args.row_hi) {
+            const int site = pf_t < L - 1 ? (L - 1 - pf_t) : (pf_t - (L - 1));
+            const double* src = env_d + ((size_t)args.slot_of_row[pf_r] * L + site) * TSZ;
+            double* dst = sT + pf_stage * TSZ;
             for (int o = tid * 2; o < TSZ; o += SAMPLE_THREADS * 2) cp_async16(dst + o, src + o);
+            if (++pf_t == steps_per_row) { pf_t = 0; ++pf_r; }
         }
+        if (++pf_stage == SAMPLE_STAGES) pf_stage = 0;
         cp_async_commit();
     };
-    for (int s = 0; s < SAMPLE_STAGES - 1; ++s) issue_prefetch(s);
+    for (int s = 0; s < SAMPLE_STAGES - 1; ++s) issue_prefetch();
 
-    long long step = 0;
     for (int r = args.row_lo; r < args.row_hi; ++r) {
         const bool has_up = r > 0;
         // ============================================================ right sweep
@@ -159,11 +160,12 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, (P <= 16 ? 2 : 1)) sample_rows
         const uint32_t* jd_neg = has_up ? args.J.row(M_JD_NEG, d, r - 1) : nullptr;
         const uint32_t* jd_nz = has_up ? args.J.row(M_JD_NZ, d, r - 1) : nullptr;
         int cur_word = -1;
-        for (int col = L - 2; col >= 0; --col, ++step) {
+        for (int col = L - 2; col >= 0; --col) {
             cp_async_wait<SAMPLE_STAGES - 2>();
             __syncthreads();
-            issue_prefetch(step + SAMPLE_STAGES - 1);
-            const double* T = sT + (size_t)(step % SAMPLE_STAGES) * TSZ;   // tensor of site col+1
+            issue_prefetch();
+            const double* T = sT + cur_stage * TSZ;   // tensor of site col+1
+            if (++cur_stage == SAMPLE_STAGES) cur_stage = 0;
             const int site = col + 1;
             if ((site >> 5) != cur_word) {
                 cur_word = site >> 5;
@@ -229,11 +231,12 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, (P <= 16 ? 2 : 1)) sample_rows
         uint32_t neww = 0;          // owner lane: bits of the current word of the new row
         uint32_t forcedw = 0;
         double prod = 1.0;          // owner lane: running product of chosen probabilities
-        for (int col = 0; col < L; ++col, ++step) {
+        for (int col = 0; col < L; ++col) {
             cp_async_wait<SAMPLE_STAGES - 2>();
             __syncthreads();
-            issue_prefetch(step + SAMPLE_STAGES - 1);
-            const double* T = sT + (size_t)(step % SAMPLE_STAGES) * TSZ;   // tensor of site col
+            issue_prefetch();
+            const double* T = sT + cur_stage * TSZ;   // tensor of site col
+            if (++cur_stage == SAMPLE_STAGES) cur_stage = 0;
             if ((col >> 5) != cur_word) {
                 cur_word = col >> 5;
                 if (has_up) {
