@@ -248,21 +248,22 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, 2) sample_rows_tf32_kernel(con
             const int jsign = has_up ? (((jnz >> bit) & 1u) ? (((jneg >> bit) & 1u) ? -1 : 1) : 0) : 0;
             int a_sel = 0;
             if (owner) {
-                double r0 = (double)rho0[0], r1 = (double)rho1[0];
+                float r0 = rho0[0], r1 = rho1[0];
                 uint32_t uw = upw[0];
 #pragma unroll
-                for (int mt = 1; mt < MT; ++mt) if (q == mt) { r0 = (double)rho0[mt]; r1 = (double)rho1[mt]; uw = upw[mt]; }
-                if (r0 == 0.0 || r1 == 0.0) {          // reading G10: count and clamp (to the smallest normal FP32)
+                for (int mt = 1; mt < MT; ++mt) if (q == mt) { r0 = rho0[mt]; r1 = rho1[mt]; uw = upw[mt]; }
+                if (r0 == 0.0f || r1 == 0.0f) {        // reading G10: count and clamp (to the smallest normal FP32)
                     if (own_active) raise_flag(args.flags, FLAG_RHO_ZERO);
-                    if (r0 == 0.0) r0 = 1.1754943508222875e-38;
-                    if (r1 == 0.0) r1 = 1.1754943508222875e-38;
+                    if (r0 == 0.0f) r0 = 1.1754943508222875e-38f;
+                    if (r1 == 0.0f) r1 = 1.1754943508222875e-38f;
                 }
                 const int t = jsign * (((uw >> bit) & 1u) ? 1 : -1);
-                const double ebd = (double)eb, embd = (double)emb;
-                const double w1 = t > 0 ? ebd : (t < 0 ? embd : 1.0);
-                const double w0 = t > 0 ? embd : (t < 0 ? ebd : 1.0);
-                const double f0 = r0 * w0, f1 = r1 * w1;
-                const double p1 = fmin(f1 * fast_rcp(f0 + f1), 1.0), p0 = 1.0 - p1;
+                const float w1 = t > 0 ? eb : (t < 0 ? emb : 1.0f);
+                const float w0 = t > 0 ? emb : (t < 0 ? eb : 1.0f);
+                // sigma(log(r1/r0) + 2 beta J s_up) = r1 w1 / (r0 w0 + r1 w1) in FP32 (r's scaled against overflow of
+                // the sum: both are <= 1 by the normalisation); p1 is then a fixed FP64 number and p0 = 1 - p1 exactly
+                const float f0 = r0 * w0, f1 = r1 * w1;
+                const double p1 = (double)fminf(__fdividef(f1, f0 + f1), 1.0f), p0 = 1.0 - p1;
                 const double u = philox_uniform((uint32_t)(r * L + col), ctr_samp, ctr_dis, TAG_SPIN,
                                                 args.seed_lo, args.seed_hi);
                 if (args.forced != nullptr) a_sel = (forcedw >> bit) & 1u;

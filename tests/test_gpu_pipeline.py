@@ -73,7 +73,7 @@ def test_exact_chi_acceptance_is_one(tn):
         assert abs(logZ[d].item() - exact.transfer_logZ(Jr[d], Jd[d], beta)) < 1e-10 * abs(logZ[d].item())
 
 
-@pytest.mark.parametrize("L,chi,k", [(12, 4, 3), (12, 4, 5), (9, 4, 1), (10, 8, 4), (8, 4, 7)])
+@pytest.mark.parametrize("L,chi,k", [(12, 4, 3), (12, 4, 5), (9, 4, 1), (10, 8, 4), (8, 4, 7), (20, 16, 6), (26, 32, 7)])
 def test_checkpoint_recompute_matches_full_stack(tn, L, chi, k):
     """a-6: the checkpoint + segment-recompute policy gives bit-identical samples and log q."""
     n_dis, n_s, beta, seed = 3, 37, 1.0, 99
