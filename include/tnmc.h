@@ -15,7 +15,8 @@
  *                    sampling sweep (Eq. 5), returning bit-packed
  *                    configurations and log q(s) (Eq. 9);
  *   tnmc_energy      Eq. 1, exact integer arithmetic;
- *   tnmc_metropolis  the independence Metropolis-Hastings acceptance of Eq. 10.
+ *   tnmc_metropolis  the independence Metropolis-Hastings acceptance of Eq. 10;
+ *   tnmc_observables thermal averages of E and M along the accepted chain.
  *
  * Conventions
  *   rows r = 0..L-1 top to bottom, columns c = 0..L-1 left to right, raster order
@@ -164,6 +165,19 @@ tnmc_status tnmc_metropolis(tnmc_ctx* ctx, int dis_begin, int dis_count, int n_s
                             uint64_t seed, uint64_t step_offset,
                             double* cur_logq, int32_t* cur_E, int64_t* cur_idx,
                             uint8_t* accepted, int64_t* n_accepted, double* sum_min1);
+
+/* Thermal averages along the Metropolis chain (the purpose of the samples; no code in the
+ * paper; reading G19 of DESIGN.md): at step n the chain sits on the last accepted proposal and every step
+ * counts once.  Per disorder the five sums over the steps of this call of  E, E^2, M, |M|, M^2  are ADDED
+ * to `sums` (M = sum_i s_i; exact integer arithmetic, converted to double once per call).
+ *   cfg_bits, E  [dev] as produced by tnmc_sample / tnmc_energy;  accepted [dev] uint8 from tnmc_metropolis
+ *   M        [dev] int32 (dis_count, n_samples)  out: magnetisation of every proposal
+ *   cur_E, cur_M [dev] int32 (dis_count)  in/out: state of the chain entering / leaving this call (read
+ *            only while no proposal of the call has been accepted yet; a fresh chain's first flag is 1)
+ *   sums     [dev] double (dis_count, 5)  in/out accumulators (zero them before the first call) */
+tnmc_status tnmc_observables(tnmc_ctx* ctx, int dis_begin, int dis_count, int n_samples,
+                             const uint32_t* cfg_bits, const int32_t* E, const uint8_t* accepted,
+                             int32_t* M, int32_t* cur_E, int32_t* cur_M, double* sums);
 
 /* One whole pass for host callers: copies Jr/Jd (host, int8 (n_dis,L,L)) to the device, builds
  * the environments, samples, computes energies, runs the Metropolis scan on fresh chains and

@@ -14,6 +14,7 @@ bmps        C0-C3 boundary-MPS cache build: Boltzmann matrices (Eq. 7), copy ten
             (Eq. 8), bottom row, row MPO, MPO x MPS, compress (reading P-C2), log Z
 sampler     S1-S2 right-environment sweep and left sampling sweep
 metropolis  S4 independence Metropolis scan (Eq. 10)
+observables thermal averages of E and M along the accepted chain (reading G19)
 philox      Part R counter-based uniforms, Philox4x32-10, indexed (disorder, sample, site)
 
 Pins (tests/test_oracle_*.py, all `-m "not gpu"`): closed forms, brute force on <=4x4,

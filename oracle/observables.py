@@ -1,0 +1,34 @@
+"""Oracle: thermal averages along the Metropolis chain (test infrastructure, see oracle/__init__.py).
+
+The paper's samples exist to estimate observables of the Boltzmann distribution (PAPER.md:23, :39:
+"unbiased samples ... physical observables"); it shows no code for this step.  Reading G19
+(DESIGN.md): the estimator is the plain MCMC average over chain STEPS -- at step n the chain sits on
+the last accepted proposal (Eq. 10; readings G15/G16), and every step counts once,
+rejected steps re-counting the state they stayed on.  Observables per configuration:
+  E   Eq. 1, integer
+  M   = sum_i s_i (magnetisation, integer in [-N, N])
+accumulated as the five sums  sum E, sum E^2, sum M, sum |M|, sum M^2  over the steps of a chunk.
+"""
+import numpy as np
+
+
+def magnetisation(cfg):
+    """M = sum_i s_i for cfg (..., L, L) in {0,1}."""
+    c = np.asarray(cfg, dtype=np.int64)
+    return (2 * c - 1).sum(axis=(-1, -2))
+
+
+def chain_sums(E, M, accepted, cur_E=0, cur_M=0):
+    """E, M: (n,) ints of the proposals; accepted: (n,) flags from the Metropolis scan (flag 1 on the
+    proposal that initialises an empty chain).  cur_E / cur_M: state entering the chunk (used until the
+    first flag 1).  Returns (sums[5] as Python ints, cur_E, cur_M)."""
+    s = [0, 0, 0, 0, 0]
+    for i in range(len(E)):
+        if accepted[i]:
+            cur_E, cur_M = int(E[i]), int(M[i])
+        s[0] += cur_E
+        s[1] += cur_E * cur_E
+        s[2] += cur_M
+        s[3] += abs(cur_M)
+        s[4] += cur_M * cur_M
+    return s, cur_E, cur_M

@@ -85,4 +85,40 @@ __global__ void metropolis_kernel(double beta, int dis_begin, int dis_count, int
     if (sum_min1 != nullptr) sum_min1[dl] = smin;
 }
 
+// Magnetisation M = sum_i s_i of every configuration (popcount on the packed words): one warp per
+// configuration, lanes stride over its L*W words.
+__global__ void magnetisation_kernel(int L, int W, long long n_cfg, const uint32_t* __restrict__ cfg,
+                                     int32_t* __restrict__ M) {
+    const long long wid = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (wid >= n_cfg) return;
+    const int lane = threadIdx.x & 31;
+    const uint32_t* s = cfg + (size_t)wid * L * W;
+    int up = 0;
+    for (int i = lane; i < L * W; i += 32) up += __popc(s[i]);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) up += __shfl_xor_sync(0xffffffffu, up, o);
+    if (lane == 0) M[wid] = 2 * up - L * L;
+}
+
+// Thermal averages along the Metropolis chain (reading G19): at step n the chain sits on the last
+// accepted proposal; every step adds E, E^2, M, |M|, M^2 of that state to the five accumulators.
+// One thread per disorder, sequential over its proposals; exact integer arithmetic in 64 bits,
+// added to the double accumulators once at the end.
+__global__ void observables_kernel(int dis_count, int n_samples, const int32_t* __restrict__ E,
+                                   const int32_t* __restrict__ M, const uint8_t* __restrict__ accepted,
+                                   int32_t* cur_E, int32_t* cur_M, double* sums) {
+    const int dl = blockIdx.x * blockDim.x + threadIdx.x;
+    if (dl >= dis_count) return;
+    long long ce = cur_E[dl], cm = cur_M[dl];
+    long long s0 = 0, s1 = 0, s2 = 0, s3 = 0, s4 = 0;
+    const size_t base = (size_t)dl * n_samples;
+    for (int n = 0; n < n_samples; ++n) {
+        if (accepted[base + n]) { ce = E[base + n]; cm = M[base + n]; }
+        s0 += ce; s1 += ce * ce; s2 += cm; s3 += cm < 0 ? -cm : cm; s4 += cm * cm;
+    }
+    cur_E[dl] = (int32_t)ce; cur_M[dl] = (int32_t)cm;
+    double* o = sums + (size_t)dl * 5;
+    o[0] += (double)s0; o[1] += (double)s1; o[2] += (double)s2; o[3] += (double)s3; o[4] += (double)s4;
+}
+
 }  // namespace tnmc

@@ -40,6 +40,8 @@ def _load():
     lib.tnmc_energy.argtypes = [vp, i32, i32, i32, vp, vp]
     lib.tnmc_metropolis.restype = i32
     lib.tnmc_metropolis.argtypes = [vp, i32, i32, i32, vp, vp, u64, u64, vp, vp, vp, vp, vp, vp]
+    lib.tnmc_observables.restype = i32
+    lib.tnmc_observables.argtypes = [vp, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp]
     lib.tnmc_run_host_workspace_bytes.restype = sz
     lib.tnmc_run_host_workspace_bytes.argtypes = [i32, i32, i32, i32, i32, i32]
     lib.tnmc_run_host.restype = i32
@@ -177,6 +179,20 @@ class Context:
                                    _ptr(cur_idx, torch.int64), _ptr(accepted, torch.uint8),
                                    _ptr(n_acc, torch.int64), _ptr(smin, torch.float64)), self.h)
         return accepted, n_acc, state, smin
+
+    def tnmc_observables(self, cfg_bits, E, accepted, dis_begin=0, state=None, sums=None):
+        """returns (M, (cur_E, cur_M), sums) -- sums (dis_count, 5) accumulates E, E^2, M, |M|, M^2 over the steps"""
+        dis_count, n_samples = E.shape
+        dev = self.device
+        if state is None:
+            state = (torch.zeros(dis_count, dtype=torch.int32, device=dev), torch.zeros(dis_count, dtype=torch.int32, device=dev))
+        if sums is None:
+            sums = torch.zeros((dis_count, 5), dtype=torch.float64, device=dev)
+        M = torch.empty((dis_count, n_samples), dtype=torch.int32, device=dev)
+        _check(lib.tnmc_observables(self.h, dis_begin, dis_count, n_samples, _ptr(cfg_bits, torch.int32), _ptr(E, torch.int32),
+                                    _ptr(accepted, torch.uint8), _ptr(M, torch.int32), _ptr(state[0], torch.int32),
+                                    _ptr(state[1], torch.int32), _ptr(sums, torch.float64)), self.h)
+        return M, state, sums
 
     # -- inspection -----------------------------------------------------------------------------
     def tnmc_get_flags(self):
