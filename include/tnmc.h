@@ -119,6 +119,27 @@ tnmc_status tnmc_create(tnmc_ctx** out, int L, int chi, double beta, int n_dis,
                         int n_samples_max, tnmc_prec prec, int ckpt_stride,
                         void* workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* Real-valued couplings (Gaussian Edwards-Anderson and any other J_ij; SURVEY 8f NEXT-1 -- Eq. 1, Eq. 7 and
+ * the whole method hold for any J_ij).  As tnmc_create, with
+ *   Jr, Jd [dev] double (n_dis, L, L), 0 on the open boundary (c = L-1 for Jr, r = L-1 for Jd); copied into the
+ *   workspace (>= tnmc_workspace_bytes_real) by a device-to-device copy enqueued on the stream.
+ * A context created this way uses tnmc_energy_real / tnmc_metropolis_real (energies are doubles);
+ * tnmc_energy returns TNMC_ESTATE on it (and tnmc_energy_real on a +-J context).  Everything else is the same. */
+size_t tnmc_workspace_bytes_real(int L, int chi, int n_dis, int n_samples_max, tnmc_prec prec, int ckpt_stride);
+tnmc_status tnmc_create_real(tnmc_ctx** out, int L, int chi, double beta, int n_dis,
+                             const double* Jr, const double* Jd, uint64_t first_disorder,
+                             int n_samples_max, tnmc_prec prec, int ckpt_stride,
+                             void* workspace, size_t workspace_bytes, void* cuda_stream);
+/* E [dev] double (dis_count, n_samples): -sum_<ij> J_ij s_i s_j in FP64, deterministic summation order. */
+tnmc_status tnmc_energy_real(tnmc_ctx* ctx, int dis_begin, int dis_count, int n_samples,
+                             const uint32_t* cfg_bits, double* E);
+/* As tnmc_metropolis with double energies (E and cur_E). */
+tnmc_status tnmc_metropolis_real(tnmc_ctx* ctx, int dis_begin, int dis_count, int n_samples,
+                                 const double* E, const double* logq,
+                                 uint64_t seed, uint64_t step_offset,
+                                 double* cur_logq, double* cur_E, int64_t* cur_idx,
+                                 uint8_t* accepted, int64_t* n_accepted, double* sum_min1);
+
 /* Build the boundary-MPS environment stack (steps a-1..a-7 of DESIGN.md).
  *   logZ [dev] double (n_dis) or NULL:  log Z_chi(d) = logscale_0 + log sum_sigma Psihat_0(sigma).
  * With ckpt_stride > 0 only the checkpoint rows are kept.  Must precede tnmc_sample. */

@@ -26,6 +26,16 @@ def energy(cfg, Jr, Jd):
     return -(e_right + e_down)
 
 
+def energy_real(cfg, Jr, Jd):
+    """E1 for real-valued couplings (Eq. 1 holds for any J_ij): float64."""
+    s = 2.0 * np.asarray(cfg, dtype=np.float64) - 1.0
+    Jr = np.asarray(Jr, dtype=np.float64)
+    Jd = np.asarray(Jd, dtype=np.float64)
+    e_right = (s[..., :, :-1] * s[..., :, 1:] * Jr[:, :-1]).sum(axis=(-1, -2))
+    e_down = (s[..., :-1, :] * s[..., 1:, :] * Jd[:-1, :]).sum(axis=(-1, -2))
+    return -(e_right + e_down)
+
+
 def all_configs(L):
     """(2^(L*L), L, L) array of every configuration, raster bit order (site 0 = MSB)."""
     n = L * L

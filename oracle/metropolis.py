@@ -29,3 +29,24 @@ def metropolis_scan(E, logq, beta, u, cur_E=0, cur_logq=0.0, cur_idx=-1, idx_off
             accepted[i] = 1
             n_acc += 1
     return accepted, n_acc, cur_E, cur_logq, cur_idx, sum_ratio
+
+
+def metropolis_scan_real(E, logq, beta, u, cur_E=0.0, cur_logq=0.0, cur_idx=-1, idx_offset=0):
+    """The same scan for real-valued energies (real couplings): Eq. 10 unchanged."""
+    n = len(E)
+    accepted = np.zeros(n, dtype=np.uint8)
+    n_acc = 0
+    sum_ratio = 0.0
+    for i in range(n):
+        if cur_idx < 0:
+            cur_E, cur_logq, cur_idx = float(E[i]), float(logq[i]), idx_offset + i
+            accepted[i] = 1
+            continue
+        logA = -beta * (float(E[i]) - cur_E) + cur_logq - float(logq[i])
+        sum_ratio += min(1.0, np.exp(min(logA, 0.0)))
+        logu = np.log(u[i]) if u[i] > 0.0 else -np.inf
+        if logu < logA:
+            cur_E, cur_logq, cur_idx = float(E[i]), float(logq[i]), idx_offset + i
+            accepted[i] = 1
+            n_acc += 1
+    return accepted, n_acc, cur_E, cur_logq, cur_idx, sum_ratio

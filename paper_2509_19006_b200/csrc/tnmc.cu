@@ -35,18 +35,19 @@ extern "C" size_t tnmc_workspace_bytes(int L, int chi, int n_dis, int n_samples_
     return p.total;
 }
 
-extern "C" tnmc_status tnmc_create(tnmc_ctx** out, int L, int chi, double beta, int n_dis,
-                                   const int8_t* Jr, const int8_t* Jd, uint64_t first_disorder,
-                                   int n_samples_max, tnmc_prec prec, int ckpt_stride,
-                                   void* workspace, size_t workspace_bytes, void* cuda_stream) {
+static tnmc_status create_impl(tnmc_ctx** out, int L, int chi, double beta, int n_dis,
+                               const int8_t* Jr, const int8_t* Jd, const double* Jr_real, const double* Jd_real,
+                               uint64_t first_disorder, int n_samples_max, tnmc_prec prec, int ckpt_stride,
+                               void* workspace, size_t workspace_bytes, void* cuda_stream) {
+    const int real_j = Jr_real != nullptr;
     if (!out) return fail(nullptr, TNMC_EINVAL, "tnmc_create: out is NULL");
     *out = nullptr;
     if (prec != TNMC_F64 && prec != TNMC_F32_LOGSCALE) return fail(nullptr, TNMC_EINVAL, "tnmc_create: unknown precision");
-    if (!Jr || !Jd || !workspace) return fail(nullptr, TNMC_EINVAL, "tnmc_create: NULL pointer");
+    if (!((Jr && Jd) || (Jr_real && Jd_real)) || !workspace) return fail(nullptr, TNMC_EINVAL, "tnmc_create: NULL pointer");
     if (!(beta >= 0.0) || !std::isfinite(beta)) return fail(nullptr, TNMC_EINVAL, "tnmc_create: beta must be finite and >= 0");
     if ((reinterpret_cast<uintptr_t>(workspace) & 255u) != 0) return fail(nullptr, TNMC_EINVAL, "tnmc_create: workspace must be 256-byte aligned");
     Plan p;
-    if (!make_plan(p, L, chi, n_dis, n_samples_max, ckpt_stride, (int)prec))
+    if (!make_plan(p, L, chi, n_dis, n_samples_max, ckpt_stride, (int)prec, real_j))
         return fail(nullptr, TNMC_EINVAL, "tnmc_create: need 2 <= L <= 4096, 2 <= chi <= 32, n_dis >= 1, n_samples_max >= 1, ckpt_stride >= 0");
     if (workspace_bytes < p.total) return fail(nullptr, TNMC_ENOMEM, "tnmc_create: workspace too small");
     int dev_count = 0;
@@ -72,7 +73,13 @@ extern "C" tnmc_status tnmc_create(tnmc_ctx** out, int L, int chi, double beta, 
     if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);   // `maps` is a host temporary
     if (e == cudaSuccess) e = cudaMemsetAsync(ctx->at<char>(p.off_flags), 0, sizeof(unsigned long long) * N_FLAGS, ctx->stream);
     if (e != cudaSuccess) return bail(cuda_fail(ctx, e, "tnmc_create: upload"));
-    {
+    if (real_j) {
+        // real couplings are kept as doubles inside the workspace (device-to-device copy on the stream)
+        const size_t nb = sizeof(double) * (size_t)n_dis * L * L;
+        e = cudaMemcpyAsync(ctx->at<double>(p.off_jreal), Jr_real, nb, cudaMemcpyDeviceToDevice, ctx->stream);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(ctx->at<char>(p.off_jreal) + nb, Jd_real, nb, cudaMemcpyDeviceToDevice, ctx->stream);
+        if (e != cudaSuccess) return bail(cuda_fail(ctx, e, "tnmc_create_real: copy"));
+    } else {
         const size_t n_words = (size_t)n_dis * L * p.W;
         const int threads = 256;
         const unsigned blocks = (unsigned)((n_words + threads - 1) / threads);
@@ -83,6 +90,30 @@ extern "C" tnmc_status tnmc_create(tnmc_ctx** out, int L, int chi, double beta, 
     }
     *out = ctx;
     return TNMC_OK;
+}
+
+extern "C" tnmc_status tnmc_create(tnmc_ctx** out, int L, int chi, double beta, int n_dis,
+                                   const int8_t* Jr, const int8_t* Jd, uint64_t first_disorder,
+                                   int n_samples_max, tnmc_prec prec, int ckpt_stride,
+                                   void* workspace, size_t workspace_bytes, void* cuda_stream) {
+    if (!Jr || !Jd) return fail(nullptr, TNMC_EINVAL, "tnmc_create: NULL pointer");
+    return create_impl(out, L, chi, beta, n_dis, Jr, Jd, nullptr, nullptr, first_disorder, n_samples_max, prec, ckpt_stride,
+                       workspace, workspace_bytes, cuda_stream);
+}
+
+extern "C" tnmc_status tnmc_create_real(tnmc_ctx** out, int L, int chi, double beta, int n_dis,
+                                        const double* Jr, const double* Jd, uint64_t first_disorder,
+                                        int n_samples_max, tnmc_prec prec, int ckpt_stride,
+                                        void* workspace, size_t workspace_bytes, void* cuda_stream) {
+    if (!Jr || !Jd) return fail(nullptr, TNMC_EINVAL, "tnmc_create_real: NULL pointer");
+    return create_impl(out, L, chi, beta, n_dis, nullptr, nullptr, Jr, Jd, first_disorder, n_samples_max, prec, ckpt_stride,
+                       workspace, workspace_bytes, cuda_stream);
+}
+
+extern "C" size_t tnmc_workspace_bytes_real(int L, int chi, int n_dis, int n_samples_max, tnmc_prec prec, int ckpt_stride) {
+    Plan p;
+    if (!make_plan(p, L, chi, n_dis, n_samples_max, ckpt_stride, (int)prec, 1)) return 0;
+    return p.total;
 }
 
 extern "C" const char* tnmc_last_error(const tnmc_ctx* ctx) { return ctx ? ctx->err.c_str() : g_err.c_str(); }
@@ -124,22 +155,30 @@ static tnmc_status launch_build(tnmc_ctx* ctx, int m, int row_hi, int row_lo, in
     return TNMC_OK;
 }
 
-template <int P, bool F32>
+template <int P, bool F32, bool REALJ>
 static cudaError_t launch_sample_t(const tnmc_ctx* ctx, const SampleArgs& a, int tiles, int dis_count) {
+    const int W = (a.L + 31) / 32;
     if (F32) {
-        const int W32 = (a.L + 31) / 32;
-        const size_t smem32 = sizeof(float) * SAMPLE_STAGES * 2 * P * P + sizeof(uint32_t) * SAMPLE_CHAINS * W32;
-        cudaError_t e32 = cudaFuncSetAttribute(sample_rows_tf32_kernel<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem32);
+        const size_t smem32 = sizeof(float) * SAMPLE_STAGES * 2 * P * P + sizeof(uint32_t) * SAMPLE_CHAINS * W +
+                              (REALJ ? sizeof(float) * 2 * a.L : 0);
+        cudaError_t e32 = cudaFuncSetAttribute(sample_rows_tf32_kernel<P, REALJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem32);
         if (e32 != cudaSuccess) return e32;
-        sample_rows_tf32_kernel<P><<<dim3(tiles, dis_count), SAMPLE_THREADS, smem32, ctx->stream>>>(a);
+        sample_rows_tf32_kernel<P, REALJ><<<dim3(tiles, dis_count), SAMPLE_THREADS, smem32, ctx->stream>>>(a);
         return cudaPeekAtLastError();
     }
-    const int W = (a.L + 31) / 32;
-    const size_t smem = sizeof(double) * SAMPLE_STAGES * 2 * P * P + sizeof(uint32_t) * SAMPLE_CHAINS * W;
-    cudaError_t e = cudaFuncSetAttribute(sample_rows_kernel<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    const size_t smem = sizeof(double) * SAMPLE_STAGES * 2 * P * P + sizeof(uint32_t) * SAMPLE_CHAINS * W +
+                        (REALJ ? sizeof(double) * 2 * a.L : 0);
+    cudaError_t e = cudaFuncSetAttribute(sample_rows_kernel<P, REALJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    sample_rows_kernel<P><<<dim3(tiles, dis_count), SAMPLE_THREADS, smem, ctx->stream>>>(a);
+    sample_rows_kernel<P, REALJ><<<dim3(tiles, dis_count), SAMPLE_THREADS, smem, ctx->stream>>>(a);
     return cudaPeekAtLastError();
+}
+template <bool F32, bool REALJ>
+static cudaError_t launch_sample_p(const tnmc_ctx* ctx, const SampleArgs& a, int tiles, int dis_count) {
+    const int P = ctx->plan.P;
+    if (P == 8) return launch_sample_t<8, F32, REALJ>(ctx, a, tiles, dis_count);
+    if (P == 16) return launch_sample_t<16, F32, REALJ>(ctx, a, tiles, dis_count);
+    return launch_sample_t<32, F32, REALJ>(ctx, a, tiles, dis_count);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -209,15 +248,8 @@ extern "C" tnmc_status tnmc_sample_ex(tnmc_ctx* ctx, int dis_begin, int dis_coun
         } else { a.row_lo = 0; a.row_hi = p.L; }
         a.slot_of_row = ctx->map(m);
         cudaError_t e;
-        if (p.f32) {
-            if (p.P == 8) e = launch_sample_t<8, true>(ctx, a, tiles, dis_count);
-            else if (p.P == 16) e = launch_sample_t<16, true>(ctx, a, tiles, dis_count);
-            else e = launch_sample_t<32, true>(ctx, a, tiles, dis_count);
-        } else {
-            if (p.P == 8) e = launch_sample_t<8, false>(ctx, a, tiles, dis_count);
-            else if (p.P == 16) e = launch_sample_t<16, false>(ctx, a, tiles, dis_count);
-            else e = launch_sample_t<32, false>(ctx, a, tiles, dis_count);
-        }
+        if (p.f32) e = p.real_j ? launch_sample_p<true, true>(ctx, a, tiles, dis_count) : launch_sample_p<true, false>(ctx, a, tiles, dis_count);
+        else e = p.real_j ? launch_sample_p<false, true>(ctx, a, tiles, dis_count) : launch_sample_p<false, false>(ctx, a, tiles, dis_count);
         if (e != cudaSuccess) return cuda_fail(ctx, e, "sample_rows_kernel");
         ctx->launches++;
     }
@@ -239,6 +271,7 @@ extern "C" tnmc_status tnmc_energy(tnmc_ctx* ctx, int dis_begin, int dis_count, 
     if (st != TNMC_OK) return st;
     if (!cfg_bits || !E) return fail(ctx, TNMC_EINVAL, "tnmc_energy: NULL pointer");
     const Plan& p = ctx->plan;
+    if (p.real_j) return fail(ctx, TNMC_ESTATE, "tnmc_energy: the context holds real couplings; use tnmc_energy_real");
     const long long n_cfg = (long long)dis_count * n_samples;
     const int warps = 8;
     const unsigned blocks = (unsigned)((n_cfg + warps - 1) / warps);
@@ -258,7 +291,40 @@ extern "C" tnmc_status tnmc_metropolis(tnmc_ctx* ctx, int dis_begin, int dis_cou
     if (!E || !logq || !cur_logq || !cur_E || !cur_idx || !accepted || !n_accepted)
         return fail(ctx, TNMC_EINVAL, "tnmc_metropolis: NULL pointer");
     const int threads = 64;
-    metropolis_kernel<<<(dis_count + threads - 1) / threads, threads, 0, ctx->stream>>>(
+    metropolis_kernel<int32_t><<<(dis_count + threads - 1) / threads, threads, 0, ctx->stream>>>(
+        ctx->beta, dis_begin, dis_count, n_samples, E, logq, (uint32_t)(seed & 0xffffffffu),
+        (uint32_t)(seed >> 32), step_offset, ctx->first_disorder, cur_logq, cur_E,
+        cur_idx, accepted, n_accepted, sum_min1);
+    CK_LAUNCH(ctx, "metropolis_kernel");
+    return TNMC_OK;
+}
+
+extern "C" tnmc_status tnmc_energy_real(tnmc_ctx* ctx, int dis_begin, int dis_count, int n_samples,
+                                        const uint32_t* cfg_bits, double* E) {
+    tnmc_status st = check_range(ctx, "tnmc_energy_real", dis_begin, dis_count, n_samples);
+    if (st != TNMC_OK) return st;
+    if (!cfg_bits || !E) return fail(ctx, TNMC_EINVAL, "tnmc_energy_real: NULL pointer");
+    const Plan& p = ctx->plan;
+    if (!p.real_j) return fail(ctx, TNMC_ESTATE, "tnmc_energy_real: the context holds +-J couplings; use tnmc_energy");
+    const long long n_cfg = (long long)dis_count * n_samples;
+    const int warps = 8;
+    energy_real_kernel<<<(unsigned)((n_cfg + warps - 1) / warps), warps * 32, 0, ctx->stream>>>(ctx->jview(), p.L, p.W, dis_begin,
+                                                                                               dis_count, n_samples, cfg_bits, E);
+    CK_LAUNCH(ctx, "energy_real_kernel");
+    return TNMC_OK;
+}
+
+extern "C" tnmc_status tnmc_metropolis_real(tnmc_ctx* ctx, int dis_begin, int dis_count, int n_samples,
+                                            const double* E, const double* logq,
+                                            uint64_t seed, uint64_t step_offset,
+                                            double* cur_logq, double* cur_E, int64_t* cur_idx,
+                                            uint8_t* accepted, int64_t* n_accepted, double* sum_min1) {
+    tnmc_status st = check_range(ctx, "tnmc_metropolis_real", dis_begin, dis_count, n_samples);
+    if (st != TNMC_OK) return st;
+    if (!E || !logq || !cur_logq || !cur_E || !cur_idx || !accepted || !n_accepted)
+        return fail(ctx, TNMC_EINVAL, "tnmc_metropolis_real: NULL pointer");
+    const int threads = 64;
+    metropolis_kernel<double><<<(dis_count + threads - 1) / threads, threads, 0, ctx->stream>>>(
         ctx->beta, dis_begin, dis_count, n_samples, E, logq, (uint32_t)(seed & 0xffffffffu),
         (uint32_t)(seed >> 32), step_offset, ctx->first_disorder, cur_logq, cur_E,
         cur_idx, accepted, n_accepted, sum_min1);

@@ -125,7 +125,7 @@ __global__ void __launch_bounds__(BuildCfg<P>::NT, BuildCfg<P>::CTAS_PER_SM) bui
             for (int t = tid; t < TSZ; t += NT) sA[t] = args.env.ld(Ain + t);
             __syncthreads();
             {   // C_a[i][k] = sum_m B_d[a][m] A[i][m][k]      (Eq. 7: B_d[a][m] = exp(beta Jd (2a-1)(2m-1)))
-                const int jd = args.J.jd(d, r, c);
+                const double jd = args.J.jdv(d, r, c);
                 const double w_same = exp(beta * jd), w_diff = exp(-beta * jd);
                 for (int t = tid; t < 2 * bl * br; t += NT) {
                     const int k = t % br, i = (t / br) % bl, a = t / (br * bl);
@@ -165,7 +165,7 @@ __global__ void __launch_bounds__(BuildCfg<P>::NT, BuildCfg<P>::CTAS_PER_SM) bui
             __syncthreads();
             PROF(1);
             // R_new[(a,y)][(rr,k)] = B_r[a][rr] R'_a[y][k] / |R_new|_F;  logscale += log |R_new|_F
-            const int jr = args.J.jr(d, r, c);
+            const double jr = args.J.jrv(d, r, c);
             const double w_same = exp(beta * jr), w_diff = exp(-beta * jr);
             double ss = 0.0;
             for (int t = tid; t < 2 * p * br; t += NT) {
@@ -356,7 +356,7 @@ __global__ void bottom_row_kernel(JView J, double beta, int L, int P, EnvRef env
     __syncthreads();
     if (threadIdx.x < 8) {
         const int l = threadIdx.x >> 2, a = (threadIdx.x >> 1) & 1, b = threadIdx.x & 1;
-        const int jr = (c == L - 1) ? 0 : J.jr(d, L - 1, c);
+        const double jr = (c == L - 1) ? 0.0 : J.jrv(d, L - 1, c);
         const double bm = exp(beta * jr * (2 * a - 1) * (2 * b - 1));
         if (c == 0) { if (l == 0) env.st(A + env_off_p(P, 0, a, b, env.f32), bm); }
         else if (c == L - 1) { if (b == 0 && l == a) env.st(A + env_off_p(P, l, a, 0, env.f32), 1.0); }

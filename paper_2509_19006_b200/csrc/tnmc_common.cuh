@@ -130,7 +130,16 @@ enum { M_JR_NEG = 0, M_JR_NZ = 1, M_JD_NEG = 2, M_JD_NZ = 3 };
 
 struct JView {
     const uint32_t* masks;
+    const double* jr_real;   // (n_dis, L, L) real-valued couplings (tnmc_create_real), else nullptr
+    const double* jd_real;
     int n_dis, L, W;
+    // coupling value as a double: the real array if there is one, else the +-1 / 0 of the masks
+    __device__ __forceinline__ double jrv(int d, int r, int c) const {
+        return jr_real ? jr_real[((size_t)d * L + r) * L + c] : (double)jr(d, r, c);
+    }
+    __device__ __forceinline__ double jdv(int d, int r, int c) const {
+        return jd_real ? jd_real[((size_t)d * L + r) * L + c] : (double)jd(d, r, c);
+    }
     __device__ __forceinline__ const uint32_t* row(int which, int d, int r) const {
         return masks + ((size_t)which * n_dis + d) * (size_t)L * W + (size_t)r * W;
     }

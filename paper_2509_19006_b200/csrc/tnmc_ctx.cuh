@@ -24,13 +24,14 @@ inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 struct Plan {
     int L = 0, chi = 0, P = 0, W = 0, n_dis = 0, n_samples_max = 0, ckpt = 0;
     int f32 = 0;                    // environment stack stored in FP32 (TNMC_F32_LOGSCALE)
+    int real_j = 0;                 // real-valued couplings kept as doubles (tnmc_create_real)
     int n_seg = 1, n_slots = 0, n_seg_slots = 0, n_maps = 1, tiles = 1;
     size_t tsz = 0;                 // doubles per site tensor
     size_t env_dis_stride = 0;      // doubles per disorder
     size_t qsz = 0;                 // doubles per site of the Q scratch
     // byte offsets into the workspace
     size_t off_masks = 0, off_maps = 0, off_flags = 0, off_logscale = 0, off_logz = 0, off_env = 0,
-           off_qbuf = 0, off_m0 = 0, off_renv = 0, total = 0;
+           off_qbuf = 0, off_m0 = 0, off_renv = 0, off_jreal = 0, total = 0;
 
     int ckpt_slot(int j) const { return j; }
     int bottom_slot() const { return n_seg; }
@@ -61,7 +62,8 @@ struct Plan {
     int seg_end(int j) const { const int h = (j + 1) * ckpt; return h < L ? h : L; }
 };
 
-inline bool make_plan(Plan& p, int L, int chi, int n_dis, int n_samples_max, int ckpt, int prec = 0) {
+inline bool make_plan(Plan& p, int L, int chi, int n_dis, int n_samples_max, int ckpt, int prec = 0, int real_j = 0) {
+    p.real_j = real_j;
     if (prec != 0 && prec != 1) return false;
     p.f32 = prec == 1;
     if (L < 2 || L > 4096 || chi < 2 || chi > 32 || n_dis < 1 || n_samples_max < 1 || ckpt < 0) return false;
@@ -89,6 +91,7 @@ inline bool make_plan(Plan& p, int L, int chi, int n_dis, int n_samples_max, int
     p.off_qbuf = o;     o = align_up(o + sizeof(double) * (size_t)n_dis * L * p.qsz);
     p.off_m0 = o;       o = align_up(o + sizeof(double) * (size_t)n_dis * 4 * p.P * p.P);
     p.off_renv = o;     o = align_up(o + sizeof(double) * (size_t)n_dis * p.tiles * L * SAMPLE_CHAINS * p.P);
+    p.off_jreal = o;    o = align_up(o + (real_j ? sizeof(double) * 2 * (size_t)n_dis * L * L : 0));
     p.total = o;
     return true;
 }
@@ -109,6 +112,8 @@ struct tnmc_ctx {
     tnmc::JView jview() const {
         tnmc::JView v;
         v.masks = at<uint32_t>(plan.off_masks);
+        v.jr_real = plan.real_j ? at<double>(plan.off_jreal) : nullptr;
+        v.jd_real = plan.real_j ? at<double>(plan.off_jreal) + (size_t)plan.n_dis * plan.L * plan.L : nullptr;
         v.n_dis = plan.n_dis; v.L = plan.L; v.W = plan.W;
         return v;
     }

@@ -43,24 +43,59 @@ __global__ void energy_kernel(JView J, int L, int W, int dis_begin, int dis_coun
     if (lane == 0) E[wid] = -acc;
 }
 
-// One thread per disorder: sequential scan over its proposals (readings G15/G16).
+// Real-valued couplings (tnmc_create_real): E = -sum_<ij> J_ij s_i s_j in FP64.  One warp per configuration;
+// lane l takes words l, l+32, ... and walks the 32 bonds of each word; the lane partial sums are combined in a
+// fixed order, so the result is deterministic (it differs from another summation order by rounding only).
+__global__ void energy_real_kernel(JView J, int L, int W, int dis_begin, int dis_count, int n_samples,
+                                   const uint32_t* __restrict__ cfg, double* __restrict__ E) {
+    const long long wid = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    const long long n_cfg = (long long)dis_count * n_samples;
+    if (wid >= n_cfg) return;
+    const int lane = threadIdx.x & 31;
+    const int d = dis_begin + (int)(wid / n_samples);
+    const uint32_t* s = cfg + (size_t)wid * L * W;
+    const double* jr = J.jr_real + (size_t)d * L * L;
+    const double* jd = J.jd_real + (size_t)d * L * L;
+    double acc = 0.0;
+    for (int i = lane; i < L * W; i += 32) {
+        const int w = i % W, r = i / W;
+        const uint32_t cur = s[i];
+        uint32_t nxt = cur >> 1;
+        if (w + 1 < W) nxt |= s[i + 1] << 31;
+        const uint32_t xr = cur ^ nxt;                                   // bit b: spins c and c+1 differ
+        const uint32_t xd = r + 1 < L ? (cur ^ s[i + W]) : 0u;          // bit b: spins (r,c) and (r+1,c) differ
+        const int nb = L - 32 * w < 32 ? L - 32 * w : 32;
+        for (int b = 0; b < nb; ++b) {
+            const int c = 32 * w + b;
+            const double a = jr[(size_t)r * L + c], bdn = jd[(size_t)r * L + c];   // 0 on the open boundary
+            acc += ((xr >> b) & 1u) ? -a : a;
+            acc += ((xd >> b) & 1u) ? -bdn : bdn;
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if (lane == 0) E[wid] = -acc;
+}
+
+// One thread per disorder: sequential scan over its proposals (readings G15/G16).  ET = int32 (+-J) or double.
+template <typename ET>
 __global__ void metropolis_kernel(double beta, int dis_begin, int dis_count, int n_samples,
-                                  const int32_t* __restrict__ E, const double* __restrict__ logq,
+                                  const ET* __restrict__ E, const double* __restrict__ logq,
                                   uint32_t seed_lo, uint32_t seed_hi, uint64_t step_offset,
                                   uint64_t first_disorder,
-                                  double* cur_logq, int32_t* cur_E, int64_t* cur_idx,
+                                  double* cur_logq, ET* cur_E, int64_t* cur_idx,
                                   uint8_t* accepted, int64_t* n_accepted, double* sum_min1) {
     const int dl = blockIdx.x * blockDim.x + threadIdx.x;
     if (dl >= dis_count) return;
     const uint32_t ctr_dis = (uint32_t)(first_disorder + (uint64_t)(dis_begin + dl));
     double cq = cur_logq[dl];
-    int ce = cur_E[dl];
+    ET ce = cur_E[dl];
     long long ci = cur_idx[dl];
     long long nacc = 0;
     double smin = 0.0;
     const size_t base = (size_t)dl * n_samples;
     for (int n = 0; n < n_samples; ++n) {
-        const int en = E[base + n];
+        const ET en = E[base + n];
         const double qn = logq[base + n];
         const uint64_t stepi = step_offset + (uint64_t)n;
         if (ci < 0) {                 // empty chain: first proposal initialises it (not counted)

@@ -65,7 +65,7 @@ __device__ __forceinline__ double quad_sum(double v) {
     return v;
 }
 
-template <int P>
+template <int P, bool REALJ>
 __global__ void __launch_bounds__(SAMPLE_THREADS, (P <= 16 ? 2 : 1)) sample_rows_kernel(const SampleArgs args) {
     constexpr int KT = P / 4;        // k tiles
     constexpr int NT = P / 4;        // n tiles (2P / 8)
@@ -79,6 +79,8 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, (P <= 16 ? 2 : 1)) sample_rows
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int g = lane >> 2, q = lane & 3;
     const int L = args.L, W = (L + 31) >> 5;
+    // real couplings: (e^{beta J}, e^{-beta J}) of the up bonds of the current row, one entry per column
+    double2* sJ = reinterpret_cast<double2*>(sBits + SAMPLE_CHAINS * W);
     const int dl = blockIdx.y;                       // local disorder index (output indexing)
     const int d = args.dis_begin + dl;               // ctx disorder index (env / J indexing)
     const int tile = blockIdx.x;
@@ -155,6 +157,14 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, (P <= 16 ? 2 : 1)) sample_rows
                     *dst = v;
                 }
         }
+        if (REALJ) {
+            __syncthreads();            // the previous row's left sweep is done with the table
+            if (has_up)
+                for (int c = tid; c < L; c += SAMPLE_THREADS) {
+                    const double bj = args.beta * args.J.jd_real[((size_t)d * L + (r - 1)) * L + c];
+                    sJ[c] = make_double2((double)exp(bj), (double)exp(-bj));
+                }
+        }
         uint32_t upw[MT] = {0u, 0u};
         uint32_t jneg = 0, jnz = 0;
         const uint32_t* jd_neg = has_up ? args.J.row(M_JD_NEG, d, r - 1) : nullptr;
@@ -195,11 +205,14 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, (P <= 16 ? 2 : 1)) sample_rows
             // weights of the up bond for the two spin values
             const int bit = site & 31;
             const int jsign = has_up ? (((jnz >> bit) & 1u) ? (((jneg >> bit) & 1u) ? -1 : 1) : 0) : 0;
+            // (e^{+beta J}, e^{-beta J}) of the up bond of this column: from the masks (+-J) or from the row table
+            double ep, em;
+            if (REALJ) { ep = has_up ? sJ[site].x : 1.0; em = has_up ? sJ[site].y : 1.0; }
+            else { ep = jsign > 0 ? eb : (jsign < 0 ? emb : 1.0); em = jsign > 0 ? emb : (jsign < 0 ? eb : 1.0); }
 #pragma unroll
             for (int mt = 0; mt < MT; ++mt) {
-                const int t = jsign * (((upw[mt] >> bit) & 1u) ? 1 : -1);
-                const double w1 = t > 0 ? eb : (t < 0 ? emb : 1.0);
-                const double w0 = t > 0 ? emb : (t < 0 ? eb : 1.0);
+                const bool up = (upw[mt] >> bit) & 1u;
+                const double w1 = up ? ep : em, w0 = up ? em : ep;     // exp(+-beta J s_up) for the new spin up / down
                 double nv[JT][2];
                 double ss = 0.0;
 #pragma unroll
@@ -280,6 +293,10 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, (P <= 16 ? 2 : 1)) sample_rows
             // owner lane: conditional probability (Eq. 5), draw, log q
             const int bit = col & 31;
             const int jsign = has_up ? (((jnz >> bit) & 1u) ? (((jneg >> bit) & 1u) ? -1 : 1) : 0) : 0;
+            // (e^{+beta J}, e^{-beta J}) of the up bond of this column: from the masks (+-J) or from the row table
+            double ep, em;
+            if (REALJ) { ep = has_up ? sJ[col].x : 1.0; em = has_up ? sJ[col].y : 1.0; }
+            else { ep = jsign > 0 ? eb : (jsign < 0 ? emb : 1.0); em = jsign > 0 ? emb : (jsign < 0 ? eb : 1.0); }
             int a_sel = 0;
             if (owner) {
                 double r0 = rho0[0], r1 = rho1[0];
@@ -291,9 +308,8 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, (P <= 16 ? 2 : 1)) sample_rows
                     if (r0 == 0.0) r0 = 2.2250738585072014e-308;
                     if (r1 == 0.0) r1 = 2.2250738585072014e-308;
                 }
-                const int t = jsign * (((uw >> bit) & 1u) ? 1 : -1);
-                const double w1 = t > 0 ? eb : (t < 0 ? emb : 1.0);
-                const double w0 = t > 0 ? emb : (t < 0 ? eb : 1.0);
+                const bool up = (uw >> bit) & 1u;
+                const double w1 = up ? ep : em, w0 = up ? em : ep;
                 // sigma(log(r1/r0) + 2 beta J s_up) = r1 w1 / (r0 w0 + r1 w1)
                 const double f0 = r0 * w0, f1 = r1 * w1;
                 const double inv = 1.0 / (f0 + f1);

@@ -33,7 +33,7 @@ __device__ __forceinline__ float quad_sumf(float v) {
     return v;
 }
 
-template <int P>
+template <int P, bool REALJ>
 __global__ void __launch_bounds__(SAMPLE_THREADS, 2) sample_rows_tf32_kernel(const SampleArgs args) {
     constexpr int KT8 = P / 8;       // k tiles (8 bond indices each)
     constexpr int NT = P / 4;        // n tiles (2P / 8)
@@ -48,6 +48,8 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, 2) sample_rows_tf32_kernel(con
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int g = lane >> 2, q = lane & 3;
     const int L = args.L, W = (L + 31) >> 5;
+    // real couplings: (e^{beta J}, e^{-beta J}) of the up bonds of the current row, one entry per column
+    float2* sJ = reinterpret_cast<float2*>(sBits + SAMPLE_CHAINS * W);
     const int dl = blockIdx.y;
     const int d = args.dis_begin + dl;
     const int tile = blockIdx.x;
@@ -115,6 +117,14 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, 2) sample_rows_tf32_kernel(con
                     *dst = make_float2((jt == 0 && q == 0) ? 1.0f : 0.0f, 0.0f);
                 }
         }
+        if (REALJ) {
+            __syncthreads();            // the previous row's left sweep is done with the table
+            if (has_up)
+                for (int c = tid; c < L; c += SAMPLE_THREADS) {
+                    const double bj = args.beta * args.J.jd_real[((size_t)d * L + (r - 1)) * L + c];
+                    sJ[c] = make_float2((float)exp(bj), (float)exp(-bj));
+                }
+        }
         uint32_t upw[MT] = {0u, 0u};
         uint32_t jneg = 0, jnz = 0;
         const uint32_t* jd_neg = has_up ? args.J.row(M_JD_NEG, d, r - 1) : nullptr;
@@ -155,11 +165,14 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, 2) sample_rows_tf32_kernel(con
             // weights of the up bond for the two spin values
             const int bit = site & 31;
             const int jsign = has_up ? (((jnz >> bit) & 1u) ? (((jneg >> bit) & 1u) ? -1 : 1) : 0) : 0;
+            // (e^{+beta J}, e^{-beta J}) of the up bond of this column: from the masks (+-J) or from the row table
+            float ep, em;
+            if (REALJ) { ep = has_up ? sJ[site].x : 1.0f; em = has_up ? sJ[site].y : 1.0f; }
+            else { ep = jsign > 0 ? eb : (jsign < 0 ? emb : 1.0f); em = jsign > 0 ? emb : (jsign < 0 ? eb : 1.0f); }
 #pragma unroll
             for (int mt = 0; mt < MT; ++mt) {
-                const int t = jsign * (((upw[mt] >> bit) & 1u) ? 1 : -1);
-                const float w1 = t > 0 ? eb : (t < 0 ? emb : 1.0f);
-                const float w0 = t > 0 ? emb : (t < 0 ? eb : 1.0f);
+                const bool up = (upw[mt] >> bit) & 1u;
+                const float w1 = up ? ep : em, w0 = up ? em : ep;     // exp(+-beta J s_up) for the new spin up / down
                 float nv[JT][2];
                 float ss = 0.0f;
 #pragma unroll
@@ -246,6 +259,10 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, 2) sample_rows_tf32_kernel(con
             // owner lane: conditional probability (Eq. 5), draw, log q -- in FP64
             const int bit = col & 31;
             const int jsign = has_up ? (((jnz >> bit) & 1u) ? (((jneg >> bit) & 1u) ? -1 : 1) : 0) : 0;
+            // (e^{+beta J}, e^{-beta J}) of the up bond of this column: from the masks (+-J) or from the row table
+            float ep, em;
+            if (REALJ) { ep = has_up ? sJ[col].x : 1.0f; em = has_up ? sJ[col].y : 1.0f; }
+            else { ep = jsign > 0 ? eb : (jsign < 0 ? emb : 1.0f); em = jsign > 0 ? emb : (jsign < 0 ? eb : 1.0f); }
             int a_sel = 0;
             if (owner) {
                 float r0 = rho0[0], r1 = rho1[0];
@@ -257,9 +274,8 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, 2) sample_rows_tf32_kernel(con
                     if (r0 == 0.0f) r0 = 1.1754943508222875e-38f;
                     if (r1 == 0.0f) r1 = 1.1754943508222875e-38f;
                 }
-                const int t = jsign * (((uw >> bit) & 1u) ? 1 : -1);
-                const float w1 = t > 0 ? eb : (t < 0 ? emb : 1.0f);
-                const float w0 = t > 0 ? emb : (t < 0 ? eb : 1.0f);
+                const bool up = (uw >> bit) & 1u;
+                const float w1 = up ? ep : em, w0 = up ? em : ep;
                 // sigma(log(r1/r0) + 2 beta J s_up) = r1 w1 / (r0 w0 + r1 w1) in FP32 (r's scaled against overflow of
                 // the sum: both are <= 1 by the normalisation); p1 is then a fixed FP64 number and p0 = 1 - p1 exactly
                 const float f0 = r0 * w0, f1 = r1 * w1;

@@ -40,6 +40,14 @@ def _load():
     lib.tnmc_energy.argtypes = [vp, i32, i32, i32, vp, vp]
     lib.tnmc_metropolis.restype = i32
     lib.tnmc_metropolis.argtypes = [vp, i32, i32, i32, vp, vp, u64, u64, vp, vp, vp, vp, vp, vp]
+    lib.tnmc_workspace_bytes_real.restype = sz
+    lib.tnmc_workspace_bytes_real.argtypes = [i32, i32, i32, i32, i32, i32]
+    lib.tnmc_create_real.restype = i32
+    lib.tnmc_create_real.argtypes = [C.POINTER(vp), i32, i32, dbl, i32, vp, vp, u64, i32, i32, i32, vp, sz, vp]
+    lib.tnmc_energy_real.restype = i32
+    lib.tnmc_energy_real.argtypes = [vp, i32, i32, i32, vp, vp]
+    lib.tnmc_metropolis_real.restype = i32
+    lib.tnmc_metropolis_real.argtypes = [vp, i32, i32, i32, vp, vp, u64, u64, vp, vp, vp, vp, vp, vp]
     lib.tnmc_observables.restype = i32
     lib.tnmc_observables.argtypes = [vp, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp]
     lib.tnmc_run_host_workspace_bytes.restype = sz
@@ -105,7 +113,9 @@ class Context:
                  ckpt_stride=0, workspace=None):
         n_dis = Jr.shape[0]
         assert Jr.shape == (n_dis, L, L) and Jd.shape == (n_dis, L, L)
-        need = tnmc_workspace_bytes(L, chi, n_dis, n_samples_max, prec, ckpt_stride)
+        self.real_j = Jr.dtype == torch.float64           # real-valued couplings -> tnmc_create_real
+        wsb = lib.tnmc_workspace_bytes_real if self.real_j else lib.tnmc_workspace_bytes
+        need = int(wsb(L, chi, n_dis, n_samples_max, prec, ckpt_stride))
         if need == 0:
             raise TnmcError(TNMC_EINVAL, "tnmc_workspace_bytes: invalid sizes")
         if workspace is None:
@@ -114,11 +124,13 @@ class Context:
         self.L, self.chi, self.beta, self.n_dis, self.n_samples_max = L, chi, float(beta), n_dis, n_samples_max
         self.W = words(L)
         self.device = Jr.device
-        self._Jr, self._Jd = Jr, Jd          # kept alive until the pack kernel has certainly run
+        self._Jr, self._Jd = Jr, Jd          # kept alive until the pack kernel / copy has certainly run
         h = C.c_void_p()
-        st = lib.tnmc_create(C.byref(h), L, chi, float(beta), n_dis, _ptr(Jr, torch.int8), _ptr(Jd, torch.int8),
-                             first_disorder, n_samples_max, prec, ckpt_stride,
-                             _ptr(workspace, torch.uint8), workspace.numel(), _stream())
+        jt = torch.float64 if self.real_j else torch.int8
+        create = lib.tnmc_create_real if self.real_j else lib.tnmc_create
+        st = create(C.byref(h), L, chi, float(beta), n_dis, _ptr(Jr, jt), _ptr(Jd, jt),
+                    first_disorder, n_samples_max, prec, ckpt_stride,
+                    _ptr(workspace, torch.uint8), workspace.numel(), _stream())
         _check(st)
         self.h = h
 
@@ -156,10 +168,11 @@ class Context:
 
     def tnmc_energy(self, cfg_bits, dis_begin=0, E=None):
         dis_count, n_samples = cfg_bits.shape[0], cfg_bits.shape[1]
+        et = torch.float64 if self.real_j else torch.int32
         if E is None:
-            E = torch.empty((dis_count, n_samples), dtype=torch.int32, device=self.device)
-        _check(lib.tnmc_energy(self.h, dis_begin, dis_count, n_samples, _ptr(cfg_bits, torch.int32),
-                               _ptr(E, torch.int32)), self.h)
+            E = torch.empty((dis_count, n_samples), dtype=et, device=self.device)
+        fn = lib.tnmc_energy_real if self.real_j else lib.tnmc_energy
+        _check(fn(self.h, dis_begin, dis_count, n_samples, _ptr(cfg_bits, torch.int32), _ptr(E, et)), self.h)
         return E
 
     def tnmc_metropolis(self, E, logq, seed, step_offset=0, dis_begin=0, state=None, want_sum_min1=False):
@@ -167,15 +180,17 @@ class Context:
         dev = self.device
         if state is None:
             state = (torch.zeros(dis_count, dtype=torch.float64, device=dev),
-                     torch.zeros(dis_count, dtype=torch.int32, device=dev),
+                     torch.zeros(dis_count, dtype=E.dtype, device=dev),
                      torch.full((dis_count,), -1, dtype=torch.int64, device=dev))
         cur_logq, cur_E, cur_idx = state
         accepted = torch.empty((dis_count, n_samples), dtype=torch.uint8, device=dev)
         n_acc = torch.empty(dis_count, dtype=torch.int64, device=dev)
         smin = torch.empty(dis_count, dtype=torch.float64, device=dev) if want_sum_min1 else None
-        _check(lib.tnmc_metropolis(self.h, dis_begin, dis_count, n_samples, _ptr(E, torch.int32),
+        et = torch.float64 if self.real_j else torch.int32
+        fn = lib.tnmc_metropolis_real if self.real_j else lib.tnmc_metropolis
+        _check(fn(self.h, dis_begin, dis_count, n_samples, _ptr(E, et),
                                    _ptr(logq, torch.float64), seed, step_offset,
-                                   _ptr(cur_logq, torch.float64), _ptr(cur_E, torch.int32),
+                                   _ptr(cur_logq, torch.float64), _ptr(cur_E, et),
                                    _ptr(cur_idx, torch.int64), _ptr(accepted, torch.uint8),
                                    _ptr(n_acc, torch.int64), _ptr(smin, torch.float64)), self.h)
         return accepted, n_acc, state, smin

@@ -21,7 +21,7 @@ def tn():
     return tnmc
 
 
-@pytest.mark.parametrize("L,chi,beta,n_dis,n_s", [(6, 2, 1.0, 3, 200), (33, 4, 0.8, 2, 150), (12, 8, 1.5, 2, 97)])
+@pytest.mark.parametrize("L,chi,beta,n_dis,n_s", [(6, 2, 1.0, 3, 200), (33, 4, 0.8, 2, 150), (12, 3, 1.5, 2, 97)])
 def test_observables_parity(tn, L, chi, beta, n_dis, n_s):
     dev = torch.device("cuda:0")
     Jr, Jd = make_couplings(L, n_dis, 640 + L)

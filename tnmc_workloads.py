@@ -34,6 +34,18 @@ def make_couplings(L, n_dis, inst_seed, p=0.5, first_disorder=0):
     return Jr, Jd
 
 
+def make_gaussian_couplings(L, n_dis, inst_seed, first_disorder=0):
+    """Gaussian Edwards-Anderson couplings J ~ N(0, 1) on every bond of the open L x L grid (SURVEY 8f
+    NEXT-1); float64 (n_dis, L, L), zero on the open boundary.  Same indexing as make_couplings."""
+    Jr = np.zeros((n_dis, L, L))
+    Jd = np.zeros((n_dis, L, L))
+    for d in range(n_dis):
+        rng = np.random.default_rng([int(inst_seed), int(first_disorder + d), int(L), 7])
+        Jr[d, :, : L - 1] = rng.standard_normal((L, L - 1))
+        Jd[d, : L - 1, :] = rng.standard_normal((L - 1, L))
+    return Jr, Jd
+
+
 def to_paper_layout(Jr, Jd):
     """(..., L, L, 4) float32 tensor (left, up, right, down) of PAPER.md:127, zeros at open edges."""
     J = np.zeros(Jr.shape + (4,), dtype=np.float32)
