@@ -33,9 +33,12 @@ WORKLOADS = {
     "C3": ("C3", None, None, 0, "configs[2] 128x128 chi=32 256x256 FP64"),
     "C4s": ("C4", 148, 200, 23, "configs[3] 512x512 chi=32, slice of 148 disorders x 200 samples, checkpoint stride 23"),
     "C5s": ("C5", 74, 128, 32, "configs[4] 1024x1024 chi=32, slice of 74 disorders x 128 samples, checkpoint stride 32"),
+    # the full configs[3] / configs[4]: disorder chunks of the same calls, one after the other in the same workspace
+    "C4": ("C4", None, None, 23, "configs[3] 512x512 chi=32, 500 disorders x 200 samples in 2 chunks of 250 disorders, checkpoint stride 23", 250),
+    "C5": ("C5", None, None, 32, "configs[4] 1024x1024 chi=32, 1000 disorders x 1000 samples in 8 chunks of 125 disorders, checkpoint stride 32", 125),
     "C5p": ("C5p", 500, 400, 32, "the paper headline setting (1024x1024, chi=8, PAPER.md:286) in FP64: slice of 500 disorders x 400 samples (one fifth of its 10^6 proposals), checkpoint stride 32"),
 }
-SLICES = ("C4s", "C5s", "C5p")      # steps of minutes: one warm-up step is enough to reach steady clocks (said in config.note)
+SLICES = ("C4s", "C5s", "C5p", "C4", "C5")   # steps of minutes to hours: --warmup is taken as given (0 allowed; said in config)
 
 
 def parse():
@@ -53,8 +56,9 @@ def parse():
 
 
 def workload(name):
-    key, n_dis, n_s, ckpt, note = WORKLOADS[name]
+    key, n_dis, n_s, ckpt, note = WORKLOADS[name][:5]
     c = dict(CONFIGS[key])
+    c["chunk"] = WORKLOADS[name][5] if len(WORKLOADS[name]) > 5 else None
     if n_dis:
         c["n_dis"] = n_dis
     if n_s:
@@ -200,11 +204,15 @@ def main_ours(args):
 
     c = workload(args.workload)
     L, chi, n_dis, n_s, ckpt = c["L"], c["chi"], c["n_dis"], c["n_samples"], c["ckpt"]
+    n_dis_total = n_dis                                   # per rank
+    if c.get("chunk"):
+        n_dis = min(c["chunk"], n_dis_total)              # buffers and contexts are sized for one chunk
+    chunks = [(c0, min(n_dis, n_dis_total - c0)) for c0 in range(0, n_dis_total, n_dis)]
     P = model.pad_chi(chi)
     betas = list(c["betas"])
     # weak scaling: every rank owns its own n_dis disorders (global indices rank*n_dis ...); no collective on the data path
-    first = shard.first_disorder(rank, n_dis)
-    Jr_np, Jd_np = make_couplings(L, n_dis, c["inst_seed"], first_disorder=first)
+    first = shard.first_disorder(rank, n_dis_total)
+    Jr_np, Jd_np = make_couplings(L, n_dis_total, c["inst_seed"], first_disorder=first)
     Jr_h, Jd_h = torch.from_numpy(Jr_np).pin_memory(), torch.from_numpy(Jd_np).pin_memory()
     Jr, Jd = Jr_h.to(dev), Jd_h.to(dev)
     prec = tnmc.TNMC_F32_LOGSCALE if args.prec == "f32" else tnmc.TNMC_F64
@@ -226,19 +234,31 @@ def main_ours(args):
     PHASES = ("build", "sample", "energy", "metropolis")
 
     def step(timed):
-        """one pass over the batch; returns (accepted, launches, phase ms dict)"""
+        """one pass over the batch (all disorder chunks, one after the other); returns (accepted, launches, phase ms dict)"""
+        acc, launches = 0, 0
+        ph = {k: 0.0 for k in PHASES}
+        for c0, nd in chunks:
+            a1, l1, p1 = step_chunk(c0, nd)
+            acc += a1
+            launches += l1
+            for k in PHASES:
+                ph[k] += p1[k]
+        return acc, launches, ph
+
+    def step_chunk(c0, nd):
         ctxs, n_accs = [None] * nb, [None] * nb
+        Jr_c, Jd_c = Jr[c0:c0 + nd], Jd[c0:c0 + nd]
 
         def run(phase, i):
             if phase == "build":
-                ctxs[i] = tnmc.Context(L, chi, betas[i], Jr, Jd, n_s, first_disorder=first, prec=prec, ckpt_stride=ckpt, workspace=ws[i])
-                ctxs[i].tnmc_build_envs(logZ[i])
+                ctxs[i] = tnmc.Context(L, chi, betas[i], Jr_c, Jd_c, n_s, first_disorder=first + c0, prec=prec, ckpt_stride=ckpt, workspace=ws[i])
+                ctxs[i].tnmc_build_envs(logZ[i][:nd])
             elif phase == "sample":
-                ctxs[i].tnmc_sample(n_s, c["seed"], cfg_bits=bits[i], logq=logq[i])
+                ctxs[i].tnmc_sample(n_s, c["seed"], cfg_bits=bits[i][:nd], logq=logq[i][:nd])
             elif phase == "energy":
-                ctxs[i].tnmc_energy(bits[i], E=E[i])
+                ctxs[i].tnmc_energy(bits[i][:nd], E=E[i][:nd])
             else:
-                _, n_accs[i], _, _ = ctxs[i].tnmc_metropolis(E[i], logq[i], c["seed"])
+                _, n_accs[i], _, _ = ctxs[i].tnmc_metropolis(E[i][:nd], logq[i][:nd], c["seed"])
 
         e = [ev() for _ in range(len(PHASES) + 1)]
         e[0].record(stream)
@@ -266,7 +286,7 @@ def main_ours(args):
         if world > 1:
             dist.barrier()
 
-    n_warm = max(args.warmup, 1 if args.workload in SLICES else 3)
+    n_warm = args.warmup if args.workload in SLICES else max(args.warmup, 3)
     for _ in range(n_warm):
         step(False)
     phases = {"build": 0.0, "sample": 0.0, "energy": 0.0, "metropolis": 0.0}
@@ -296,10 +316,14 @@ def main_ours(args):
 
         def host_pass(i):
             torch.cuda.set_device(local_rank)
+            tot = 0
             with torch.cuda.stream(streams[i]):
-                outs[i] = tnmc.tnmc_run_host(L, chi, betas[i], Jr_h, Jd_h, n_s, c["seed"], ws[i], first_disorder=first,
-                                             prec=prec, ckpt_stride=ckpt, out=outs[i])
-            return int(outs[i]["n_accepted"].sum().item())
+                for c0, nd in chunks:
+                    outs[i] = tnmc.tnmc_run_host(L, chi, betas[i], Jr_h[c0:c0 + nd], Jd_h[c0:c0 + nd], n_s, c["seed"], ws[i],
+                                                 first_disorder=first + c0, prec=prec, ckpt_stride=ckpt,
+                                                 out=outs[i] if len(chunks) == 1 or nd == n_dis else None)
+                    tot += int(outs[i]["n_accepted"].sum().item())
+            return tot
 
         with ThreadPoolExecutor(max_workers=nb) as pool:
             for _ in range(1 if args.workload in SLICES else 2):
@@ -313,14 +337,14 @@ def main_ours(args):
             dt = time.perf_counter() - t0
         dt_max, e_acc_sum = shard.reduce_job(dt, e_acc, dev)
         h2d = nb * (Jr_h.numel() + Jd_h.numel())
-        d2h = sum(v.numel() * v.element_size() for o in outs for v in o.values() if v is not None)
+        d2h = len(chunks) * sum(v.numel() * v.element_size() for o in outs for v in o.values() if v is not None)
         e2e = {"value": e_acc_sum / dt_max, "unit": "samples/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h}
 
     if rank == 0:
         # the nb launches of a phase run concurrently: duration of the group, algorithmic work of the group
         build_ms = phases["build"] / args.steps
         sample_ms = phases["sample"] / args.steps
-        build_flops = nb * model.build_flops_per_disorder(L, chi) * n_dis * (2.0 if ckpt else 1.0)
+        build_flops = nb * model.build_flops_per_disorder(L, chi) * n_dis_total * (2.0 if ckpt else 1.0)
         peak_dmma = tnmc.tnmc_fp64_peak_tflops(1)
         peak_dfma = tnmc.tnmc_fp64_peak_tflops(0)
         peaks = {}
@@ -329,10 +353,15 @@ def main_ours(args):
         except Exception:
             pass
         hbm_peak = peaks.get("hbm_gbs", 6650.0)
-        samp_flops = nb * model.sample_flops_per_chain_site(P) * n_dis * n_s * L * L
+        samp_flops = nb * model.sample_flops_per_chain_site(P) * n_dis_total * n_s * L * L
         w_env = 4 if args.prec == "f32" else 8
-        samp_bytes = nb * model.sample_bytes_per_chain_site(P, w=w_env) * n_dis * n_s * L * L
-        dominant = "build_rows_kernel" if phases["build"] >= phases["sample"] else "sample_rows_kernel"
+        samp_bytes = nb * model.sample_bytes_per_chain_site(P, w=w_env) * n_dis_total * n_s * L * L
+        if ckpt:
+            # checkpoint mode: tnmc_sample recomputes every segment with build_rows_kernel before sampling it, so the
+            # sample phase holds a second full build pass; the build kernel's time is taken as build + sample phase
+            # (an upper bound: it includes the sampler's own share) against the flops of both passes
+            build_ms += sample_ms
+        dominant = "build_rows_kernel" if (ckpt or phases["build"] >= phases["sample"]) else "sample_rows_kernel"
         traffic = None                                       # DRAM bytes per launch from the committed ncu capture (profiles/)
         try:
             traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(args.workload, {}).get(dominant)
@@ -363,12 +392,12 @@ def main_ours(args):
         line = {"metric": "accepted samples/s", "value": value, "unit": "samples/s", "n_gpus": world, "steps": args.steps,
                 "warmup": n_warm, "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f64" if args.prec == "f64" else "f64 compression + tf32 sampling (fp32 stack)", "data": "synthetic",
-                "config": {"workload": args.workload, "note": c["note"], "L": L, "chi": chi, "betas": betas, "n_dis_per_gpu": n_dis,
+                "config": {"workload": args.workload, "note": c["note"], "L": L, "chi": chi, "betas": betas, "n_dis_per_gpu": n_dis_total, "disorder_chunks": len(chunks),
                            "n_samples": n_s, "ckpt_stride": ckpt, "parallelism": f"dp{world} (disorders sharded, no collective)",
                            "l2": "flushed (256 MiB memset) between timed steps; env stack > L2",
                            "streams": f"{nb} (one per beta; the launches of each phase run concurrently)"},
-                "proposals_per_s": len(betas) * args.steps * n_dis * n_s * world / (ms_total * 1e-3),
-                "p_acc": acc_total / (len(betas) * args.steps * n_dis * (n_s - 1) * world),
+                "proposals_per_s": len(betas) * args.steps * n_dis_total * n_s * world / (ms_total * 1e-3),
+                "p_acc": acc_total / (len(betas) * args.steps * n_dis_total * (n_s - 1) * world),
                 "phase_ms_per_step": {k: v / args.steps for k, v in phases.items()},
                 "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": tot_launch, "clocks": clk.summary()}
         print(json.dumps(line))
