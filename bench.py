@@ -22,7 +22,7 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-from tnmc_workloads import CONFIGS, make_couplings  # noqa: E402
+from tnmc_workloads import CONFIGS, make_couplings, make_gaussian_couplings  # noqa: E402
 
 # name -> (config key, n_dis, n_samples, ckpt_stride, note).  C2 (BASELINE.json configs[1]) is the
 # default; C3 is configs[2]; C4s / C5s are disorder x sample SLICES of configs[3] / configs[4] sized to
@@ -50,6 +50,8 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--prec", default="f64", choices=["f64", "f32"],
                     help="f64: the parity path; f32: TNMC_F32_LOGSCALE (FP32 stack, TF32 tensor-core sampler, FP64 compression)")
+    ap.add_argument("--couplings", default="pmj", choices=["pmj", "gaussian"],
+                    help="pmj: +-J (the BASELINE configs); gaussian: J ~ N(0,1) through tnmc_create_real (no e2e / cpu_baseline leg)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -212,7 +214,11 @@ def main_ours(args):
     betas = list(c["betas"])
     # weak scaling: every rank owns its own n_dis disorders (global indices rank*n_dis ...); no collective on the data path
     first = shard.first_disorder(rank, n_dis_total)
-    Jr_np, Jd_np = make_couplings(L, n_dis_total, c["inst_seed"], first_disorder=first)
+    real_j = args.couplings == "gaussian"
+    if real_j:
+        args.no_e2e = args.no_cpu_baseline = True          # tnmc_run_host and the timed oracle leg are +-J only
+    gen = make_gaussian_couplings if real_j else make_couplings
+    Jr_np, Jd_np = gen(L, n_dis_total, c["inst_seed"], first_disorder=first)
     Jr_h, Jd_h = torch.from_numpy(Jr_np).pin_memory(), torch.from_numpy(Jd_np).pin_memory()
     Jr, Jd = Jr_h.to(dev), Jd_h.to(dev)
     prec = tnmc.TNMC_F32_LOGSCALE if args.prec == "f32" else tnmc.TNMC_F64
@@ -227,7 +233,7 @@ def main_ours(args):
     ws = [torch.empty(max(need, need_h), dtype=torch.uint8, device=dev) for _ in betas]
     bits = [torch.empty((n_dis, n_s, L, W), dtype=torch.int32, device=dev) for _ in betas]
     logq = [torch.empty((n_dis, n_s), dtype=torch.float64, device=dev) for _ in betas]
-    E = [torch.empty((n_dis, n_s), dtype=torch.int32, device=dev) for _ in betas]
+    E = [torch.empty((n_dis, n_s), dtype=torch.float64 if real_j else torch.int32, device=dev) for _ in betas]
     logZ = [torch.empty(n_dis, dtype=torch.float64, device=dev) for _ in betas]
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
     ev = lambda: torch.cuda.Event(enable_timing=True)
@@ -392,7 +398,7 @@ def main_ours(args):
         line = {"metric": "accepted samples/s", "value": value, "unit": "samples/s", "n_gpus": world, "steps": args.steps,
                 "warmup": n_warm, "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f64" if args.prec == "f64" else "f64 compression + tf32 sampling (fp32 stack)", "data": "synthetic",
-                "config": {"workload": args.workload, "note": c["note"], "L": L, "chi": chi, "betas": betas, "n_dis_per_gpu": n_dis_total, "disorder_chunks": len(chunks),
+                "config": {"workload": args.workload, "couplings": args.couplings, "note": c["note"], "L": L, "chi": chi, "betas": betas, "n_dis_per_gpu": n_dis_total, "disorder_chunks": len(chunks),
                            "n_samples": n_s, "ckpt_stride": ckpt, "parallelism": f"dp{world} (disorders sharded, no collective)",
                            "l2": "flushed (256 MiB memset) between timed steps; env stack > L2",
                            "streams": f"{nb} (one per beta; the launches of each phase run concurrently)"},

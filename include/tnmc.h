@@ -200,6 +200,12 @@ tnmc_status tnmc_observables(tnmc_ctx* ctx, int dis_begin, int dis_count, int n_
                              const uint32_t* cfg_bits, const int32_t* E, const uint8_t* accepted,
                              int32_t* M, int32_t* cur_E, int32_t* cur_M, double* sums);
 
+/* As tnmc_observables for a context with real couplings: E and cur_E are doubles, the sums of E and E^2 are
+ * FP64 sums in proposal order. */
+tnmc_status tnmc_observables_real(tnmc_ctx* ctx, int dis_begin, int dis_count, int n_samples,
+                                  const uint32_t* cfg_bits, const double* E, const uint8_t* accepted,
+                                  int32_t* M, double* cur_E, int32_t* cur_M, double* sums);
+
 /* One whole pass for host callers: copies Jr/Jd (host, int8 (n_dis,L,L)) to the device, builds
  * the environments, samples, computes energies, runs the Metropolis scan on fresh chains and
  * copies the results back.  All device memory comes from `workspace`

@@ -32,3 +32,17 @@ def chain_sums(E, M, accepted, cur_E=0, cur_M=0):
         s[3] += abs(cur_M)
         s[4] += cur_M * cur_M
     return s, cur_E, cur_M
+
+
+def chain_sums_real(E, M, accepted, cur_E=0.0, cur_M=0):
+    """As chain_sums for real-valued energies (real couplings): sums of E and E^2 as floats in proposal order."""
+    s = [0.0, 0.0, 0, 0, 0]
+    for i in range(len(E)):
+        if accepted[i]:
+            cur_E, cur_M = float(E[i]), int(M[i])
+        s[0] += cur_E
+        s[1] += cur_E * cur_E
+        s[2] += cur_M
+        s[3] += abs(cur_M)
+        s[4] += cur_M * cur_M
+    return s, cur_E, cur_M

@@ -332,23 +332,36 @@ extern "C" tnmc_status tnmc_metropolis_real(tnmc_ctx* ctx, int dis_begin, int di
     return TNMC_OK;
 }
 
-extern "C" tnmc_status tnmc_observables(tnmc_ctx* ctx, int dis_begin, int dis_count, int n_samples,
-                                        const uint32_t* cfg_bits, const int32_t* E, const uint8_t* accepted,
-                                        int32_t* M, int32_t* cur_E, int32_t* cur_M, double* sums) {
-    tnmc_status st = check_range(ctx, "tnmc_observables", dis_begin, dis_count, n_samples);
+template <typename ET>
+static tnmc_status observables_impl(tnmc_ctx* ctx, const char* who, int dis_begin, int dis_count, int n_samples,
+                                    const uint32_t* cfg_bits, const ET* E, const uint8_t* accepted,
+                                    int32_t* M, ET* cur_E, int32_t* cur_M, double* sums) {
+    tnmc_status st = check_range(ctx, who, dis_begin, dis_count, n_samples);
     if (st != TNMC_OK) return st;
     if (!cfg_bits || !E || !accepted || !M || !cur_E || !cur_M || !sums)
-        return fail(ctx, TNMC_EINVAL, "tnmc_observables: NULL pointer");
+        return fail(ctx, TNMC_EINVAL, std::string(who) + ": NULL pointer");
     const Plan& p = ctx->plan;
     const long long n_cfg = (long long)dis_count * n_samples;
     const int warps = 8;
     magnetisation_kernel<<<(unsigned)((n_cfg + warps - 1) / warps), warps * 32, 0, ctx->stream>>>(p.L, p.W, n_cfg, cfg_bits, M);
     CK_LAUNCH(ctx, "magnetisation_kernel");
     const int threads = 64;
-    observables_kernel<<<(dis_count + threads - 1) / threads, threads, 0, ctx->stream>>>(dis_count, n_samples, E, M, accepted,
-                                                                                        cur_E, cur_M, sums);
+    observables_kernel<ET><<<(dis_count + threads - 1) / threads, threads, 0, ctx->stream>>>(dis_count, n_samples, E, M, accepted,
+                                                                                            cur_E, cur_M, sums);
     CK_LAUNCH(ctx, "observables_kernel");
     return TNMC_OK;
+}
+
+extern "C" tnmc_status tnmc_observables(tnmc_ctx* ctx, int dis_begin, int dis_count, int n_samples,
+                                        const uint32_t* cfg_bits, const int32_t* E, const uint8_t* accepted,
+                                        int32_t* M, int32_t* cur_E, int32_t* cur_M, double* sums) {
+    return observables_impl<int32_t>(ctx, "tnmc_observables", dis_begin, dis_count, n_samples, cfg_bits, E, accepted, M, cur_E, cur_M, sums);
+}
+
+extern "C" tnmc_status tnmc_observables_real(tnmc_ctx* ctx, int dis_begin, int dis_count, int n_samples,
+                                             const uint32_t* cfg_bits, const double* E, const uint8_t* accepted,
+                                             int32_t* M, double* cur_E, int32_t* cur_M, double* sums) {
+    return observables_impl<double>(ctx, "tnmc_observables_real", dis_begin, dis_count, n_samples, cfg_bits, E, accepted, M, cur_E, cur_M, sums);
 }
 
 // ---------------------------------------------------------------------------------------------

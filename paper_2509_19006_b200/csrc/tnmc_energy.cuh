@@ -1,6 +1,8 @@
 // tnmc_energy.cuh -- exact +-J energy (a-10, Eq. 1) and the independence
 // Metropolis scan (a-11, Eq. 10).
 #pragma once
+#include <type_traits>
+
 #include "tnmc_common.cuh"
 
 namespace tnmc {
@@ -139,19 +141,22 @@ __global__ void magnetisation_kernel(int L, int W, long long n_cfg, const uint32
 // accepted proposal; every step adds E, E^2, M, |M|, M^2 of that state to the five accumulators.
 // One thread per disorder, sequential over its proposals; exact integer arithmetic in 64 bits,
 // added to the double accumulators once at the end.
-__global__ void observables_kernel(int dis_count, int n_samples, const int32_t* __restrict__ E,
+template <typename ET>
+__global__ void observables_kernel(int dis_count, int n_samples, const ET* __restrict__ E,
                                    const int32_t* __restrict__ M, const uint8_t* __restrict__ accepted,
-                                   int32_t* cur_E, int32_t* cur_M, double* sums) {
+                                   ET* cur_E, int32_t* cur_M, double* sums) {
     const int dl = blockIdx.x * blockDim.x + threadIdx.x;
     if (dl >= dis_count) return;
-    long long ce = cur_E[dl], cm = cur_M[dl];
-    long long s0 = 0, s1 = 0, s2 = 0, s3 = 0, s4 = 0;
+    // +-J: exact 64-bit integer sums; real couplings: FP64 sums in proposal order
+    typedef typename std::conditional<std::is_same<ET, int32_t>::value, long long, double>::type AT;
+    AT ce = cur_E[dl], s0 = 0, s1 = 0;
+    long long cm = cur_M[dl], s2 = 0, s3 = 0, s4 = 0;
     const size_t base = (size_t)dl * n_samples;
     for (int n = 0; n < n_samples; ++n) {
         if (accepted[base + n]) { ce = E[base + n]; cm = M[base + n]; }
         s0 += ce; s1 += ce * ce; s2 += cm; s3 += cm < 0 ? -cm : cm; s4 += cm * cm;
     }
-    cur_E[dl] = (int32_t)ce; cur_M[dl] = (int32_t)cm;
+    cur_E[dl] = (ET)ce; cur_M[dl] = (int32_t)cm;
     double* o = sums + (size_t)dl * 5;
     o[0] += (double)s0; o[1] += (double)s1; o[2] += (double)s2; o[3] += (double)s3; o[4] += (double)s4;
 }

@@ -50,6 +50,8 @@ def _load():
     lib.tnmc_metropolis_real.argtypes = [vp, i32, i32, i32, vp, vp, u64, u64, vp, vp, vp, vp, vp, vp]
     lib.tnmc_observables.restype = i32
     lib.tnmc_observables.argtypes = [vp, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp]
+    lib.tnmc_observables_real.restype = i32
+    lib.tnmc_observables_real.argtypes = [vp, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp]
     lib.tnmc_run_host_workspace_bytes.restype = sz
     lib.tnmc_run_host_workspace_bytes.argtypes = [i32, i32, i32, i32, i32, i32]
     lib.tnmc_run_host.restype = i32
@@ -200,12 +202,14 @@ class Context:
         dis_count, n_samples = E.shape
         dev = self.device
         if state is None:
-            state = (torch.zeros(dis_count, dtype=torch.int32, device=dev), torch.zeros(dis_count, dtype=torch.int32, device=dev))
+            state = (torch.zeros(dis_count, dtype=E.dtype, device=dev), torch.zeros(dis_count, dtype=torch.int32, device=dev))
         if sums is None:
             sums = torch.zeros((dis_count, 5), dtype=torch.float64, device=dev)
         M = torch.empty((dis_count, n_samples), dtype=torch.int32, device=dev)
-        _check(lib.tnmc_observables(self.h, dis_begin, dis_count, n_samples, _ptr(cfg_bits, torch.int32), _ptr(E, torch.int32),
-                                    _ptr(accepted, torch.uint8), _ptr(M, torch.int32), _ptr(state[0], torch.int32),
+        et = torch.float64 if self.real_j else torch.int32
+        fn = lib.tnmc_observables_real if self.real_j else lib.tnmc_observables
+        _check(fn(self.h, dis_begin, dis_count, n_samples, _ptr(cfg_bits, torch.int32), _ptr(E, et),
+                                    _ptr(accepted, torch.uint8), _ptr(M, torch.int32), _ptr(state[0], et),
                                     _ptr(state[1], torch.int32), _ptr(sums, torch.float64)), self.h)
         return M, state, sums
 

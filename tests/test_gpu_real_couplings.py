@@ -5,7 +5,7 @@ limit, checkpoint mode, and the reduced-precision mode's invariants."""
 import numpy as np
 import pytest
 
-from oracle import bmps, exact, metropolis, philox, sampler
+from oracle import bmps, exact, metropolis, observables, philox, sampler
 from tnmc_workloads import make_gaussian_couplings
 
 from bitpack import pack, unpack
@@ -74,6 +74,14 @@ def test_real_couplings_parity(tn, L, chi, beta, n_dis, n_s, k):
         assert (acc_h[d] == o_acc).all() and int(n_acc[d]) == o_n
         assert float(state[1][d]) == cE and int(state[2][d]) == ci
         assert abs(float(smin[d]) - sm) < 1e-9 * max(1.0, sm)
+    # observables along the chain with real energies
+    M, st_o, sums = ctx.tnmc_observables(bits, E, acc)
+    M_h, sums_h = M.cpu().numpy(), sums.cpu().numpy()
+    for d in range(n_dis):
+        assert (M_h[d] == observables.magnetisation(cfg[d])).all()
+        so, cE, cM = observables.chain_sums_real(E_h[d], M_h[d], acc_h[d])
+        assert np.allclose(sums_h[d], so, rtol=1e-12, atol=1e-9)
+        assert float(st_o[0][d]) == cE and int(st_o[1][d]) == cM
 
 
 def test_real_couplings_exact_chi_and_f32_invariants(tn):

@@ -35,6 +35,15 @@ def test_chain_sums_hand_worked():
     assert s3 == [-6, 36, -4, 4, 16]
 
 
+def test_chain_sums_real_reduces_to_integer_version():
+    E = [-4, -2, -6, -4, -4]; M = [2, 0, -4, 6, 2]; acc = [1, 0, 1, 1, 1]
+    s, cE, cM = observables.chain_sums(E, M, acc)
+    sr, cEr, cMr = observables.chain_sums_real([float(e) for e in E], M, acc)
+    assert sr == [float(s[0]), float(s[1]), s[2], s[3], s[4]] and (cEr, cMr) == (float(cE), cM)
+    sh, _, _ = observables.chain_sums_real([0.5, -1.25], [1, -3], [1, 1])
+    assert sh == [-0.75, 0.25 + 1.5625, -2, 4, 10]
+
+
 def test_exact_chi_chain_reproduces_boltzmann_averages():
     L, chi, beta, n_s, seed = 3, 8, 0.8, 6000, 21
     Jr, Jd = make_couplings(L, 1, 77)
