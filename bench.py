@@ -223,6 +223,8 @@ def main_ours(args):
     Jr, Jd = Jr_h.to(dev), Jd_h.to(dev)
     prec = tnmc.TNMC_F32_LOGSCALE if args.prec == "f32" else tnmc.TNMC_F64
     need = tnmc.tnmc_workspace_bytes(L, chi, n_dis, n_s, prec=prec, ckpt_stride=ckpt)
+    if real_j:
+        need = int(tnmc.lib.tnmc_workspace_bytes_real(L, chi, n_dis, n_s, prec, ckpt))
     need_h = tnmc.tnmc_run_host_workspace_bytes(L, chi, n_dis, n_s, prec=prec, ckpt_stride=ckpt)
     W = tnmc.words(L)
     nb = len(betas)
