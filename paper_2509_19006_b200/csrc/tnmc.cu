@@ -187,8 +187,6 @@ static cudaError_t launch_sample_p(const tnmc_ctx* ctx, const SampleArgs& a, int
 extern "C" tnmc_status tnmc_build_envs(tnmc_ctx* ctx, double* logZ) {
     if (!ctx) return fail(nullptr, TNMC_EINVAL, "tnmc_build_envs: ctx is NULL");
     const Plan& p = ctx->plan;
-    const int* map0 = ctx->map(0);
-    (void)map0;
     bottom_row_kernel<<<dim3(p.L, p.n_dis), 64, 0, ctx->stream>>>(
         ctx->jview(), ctx->beta, p.L, p.P, ctx->env(), p.env_dis_stride,
         p.perm_slot(p.L - 1), ctx->at<double>(p.off_logscale));

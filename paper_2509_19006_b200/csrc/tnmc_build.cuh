@@ -51,10 +51,7 @@ template <int P>
 struct BuildCfg {
     static constexpr int NT = 8 * P;          // threads per CTA: one quad per column of a 2P-column matrix
     static constexpr int D = 2 * P;           // doubled bond
-#ifndef TNMC_LPP
-#define TNMC_LPP 8
-#endif
-    static constexpr int LPP = TNMC_LPP;      // lanes per row pair in the Jacobi
+    static constexpr int LPP = 8;             // lanes per row pair in the Jacobi (8 measured best at chi = 16 and 32, 4 and 2 slower)
     static constexpr int LDX = D + 4;         // column-major leading dim (= 4 mod 16: a half-warp of 4 quads hits 16 distinct 8-byte banks)
     static constexpr int LDM = D + 2;         // row length of the Jacobi operand (row-major)
     static constexpr int LDV = D + 1;         // row length of the selected right singular vectors

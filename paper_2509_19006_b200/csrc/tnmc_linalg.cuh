@@ -34,9 +34,6 @@ __device__ __forceinline__ double block_sum(double v, double* scratch) {
 // ~1 ulp at the end).  x must be finite, normal and (for rsqrt) positive -- true for every squared
 // norm and pivot that reaches them (zeros are excluded by the callers).
 __device__ __forceinline__ double fast_rsqrt(double x) {
-#ifdef TNMC_SLOW_MATH
-    return rsqrt(x);
-#endif
     double r;
     asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
     const double hx = 0.5 * x;
@@ -45,9 +42,6 @@ __device__ __forceinline__ double fast_rsqrt(double x) {
     return r;
 }
 __device__ __forceinline__ double fast_rcp(double x) {
-#ifdef TNMC_SLOW_MATH
-    return 1.0 / x;
-#endif
     double r;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
     r = fma(r, fma(-x, r, 1.0), r);
