@@ -71,7 +71,7 @@ typedef enum {
 
 typedef enum {
     TNMC_F64 = 0,          /* FP64 storage and arithmetic: the parity path (log Z 1e-10, conditionals 1e-9) */
-    TNMC_F32_LOGSCALE = 1  /* reduced precision (BASELINE configs[2]; the paper's own dtype is torch.float):
+    TNMC_F32_LOGSCALE = 1, /* reduced precision (BASELINE configs[2]; the paper's own dtype is torch.float):
                               environment stack stored in FP32 -- every stored row has unit 2-norm and carries
                               its log-scale separately (reading G7), so single precision has no range problem --
                               and sampling contractions on TF32 tensor cores (mma.sync.m16n8k8, FP32 accumulate,
@@ -83,6 +83,12 @@ typedef enum {
                               (north_star reduced-precision tolerance 1e-4); conditionals carry ~1e-3 of TF32
                               noise, spins are not bit-identical to the FP64 path, the acceptance is lower.
                               TNMC_FLAG_RHO_ZERO is informational in this mode. */
+    TNMC_F32_STORE = 2     /* environment stack stored in FP32 (in the FP64 sampler's fragment order), ALL arithmetic
+                              FP64: the tensors are rounded to FP32 once when a row is stored, the compression and
+                              the FP64 DMMA sampler read them back as doubles.  Half the HBM footprint and stack
+                              traffic at conditionals within ~1e-6 of TNMC_F64 and an unchanged acceptance; spins
+                              are not bit-identical to TNMC_F64.  q is normalised and log q is the log of the
+                              probabilities used, as in every mode. */
 } tnmc_prec;
 
 /* indices into the array returned by tnmc_get_flags */

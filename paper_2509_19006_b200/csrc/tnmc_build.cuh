@@ -99,7 +99,7 @@ __global__ void __launch_bounds__(BuildCfg<P>::NT, BuildCfg<P>::CTAS_PER_SM) bui
     const int half = tid >= HALF ? 1 : 0, gt = tid - half * HALF;
     const int d = args.dis_begin + blockIdx.x;
     const int L = args.L, chi = args.chi;
-    const int f32 = args.env.f32;        // selects the fragment order of the stored tensors
+    const int f32 = args.env.lay32;      // selects the fragment order of the stored tensors
     const double beta = args.beta;
     const size_t env_d = (size_t)d * args.env_dis_stride;
     double* qbuf_d = args.qbuf + (size_t)d * (size_t)L * Cfg::QSZ;
@@ -355,9 +355,9 @@ __global__ void bottom_row_kernel(JView J, double beta, int L, int P, EnvRef env
         const int l = threadIdx.x >> 2, a = (threadIdx.x >> 1) & 1, b = threadIdx.x & 1;
         const double jr = (c == L - 1) ? 0.0 : J.jrv(d, L - 1, c);
         const double bm = exp(beta * jr * (2 * a - 1) * (2 * b - 1));
-        if (c == 0) { if (l == 0) env.st(A + env_off_p(P, 0, a, b, env.f32), bm); }
-        else if (c == L - 1) { if (b == 0 && l == a) env.st(A + env_off_p(P, l, a, 0, env.f32), 1.0); }
-        else if (l == a) env.st(A + env_off_p(P, l, a, b, env.f32), bm);
+        if (c == 0) { if (l == 0) env.st(A + env_off_p(P, 0, a, b, env.lay32), bm); }
+        else if (c == L - 1) { if (b == 0 && l == a) env.st(A + env_off_p(P, l, a, 0, env.lay32), 1.0); }
+        else if (l == a) env.st(A + env_off_p(P, l, a, b, env.lay32), bm);
     }
     if (c == 0 && threadIdx.x == 0) logscale[(size_t)d * L + (L - 1)] = 0.0;
 }
@@ -382,7 +382,7 @@ __global__ void logz_kernel(int L, int chi, int P, int n_dis, EnvRef env, size_t
         double acc = 0.0;
         for (int i = 0; i < bl; ++i) {
             const double vi = __shfl_sync(0xffffffffu, v, i);
-            if (lane < br) acc += vi * (env.ld(A + env_off_p(P, i, 0, lane, env.f32)) + env.ld(A + env_off_p(P, i, 1, lane, env.f32)));
+            if (lane < br) acc += vi * (env.ld(A + env_off_p(P, i, 0, lane, env.lay32)) + env.ld(A + env_off_p(P, i, 1, lane, env.lay32)));
         }
         double mx = fabs(acc);
 #pragma unroll
@@ -428,7 +428,7 @@ __global__ void export_row_kernel(int L, int chi, int P, EnvRef env, size_t row,
     const int TSZ = 2 * P * P;
     for (int t = threadIdx.x; t < chi * 2 * chi; t += blockDim.x) {
         const int j = t % chi, a = (t / chi) & 1, i = t / (2 * chi);
-        out[(size_t)c * chi * 2 * chi + t] = env.ld(row + (size_t)c * TSZ + env_off_p(P, i, a, j, env.f32));
+        out[(size_t)c * chi * 2 * chi + t] = env.ld(row + (size_t)c * TSZ + env_off_p(P, i, a, j, env.lay32));
     }
 }
 

@@ -65,7 +65,8 @@ __host__ __device__ __forceinline__ int env_off_p(int P, int i, int a, int j, in
 // in elements either way.
 struct EnvRef {
     void* base;
-    int f32;
+    int f32;      // element type: float (TNMC_F32_LOGSCALE, TNMC_F32_STORE) or double
+    int lay32;    // fragment order: env_off32 (TF32 sampler) or env_off (FP64 DMMA sampler)
     __device__ __forceinline__ double ld(size_t i) const {
         return f32 ? (double)reinterpret_cast<const float*>(base)[i] : reinterpret_cast<const double*>(base)[i];
     }

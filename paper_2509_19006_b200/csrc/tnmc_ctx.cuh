@@ -23,7 +23,8 @@ inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 //              the ping-pong pair of the first pass).  Segment j = rows [jk, min((j+1)k, L)).
 struct Plan {
     int L = 0, chi = 0, P = 0, W = 0, n_dis = 0, n_samples_max = 0, ckpt = 0;
-    int f32 = 0;                    // environment stack stored in FP32 (TNMC_F32_LOGSCALE)
+    int f32 = 0;                    // environment stack stored in FP32 (TNMC_F32_LOGSCALE, TNMC_F32_STORE)
+    int tf32 = 0;                   // TF32 tensor-core sampler and its fragment order (TNMC_F32_LOGSCALE)
     int real_j = 0;                 // real-valued couplings kept as doubles (tnmc_create_real)
     int n_seg = 1, n_slots = 0, n_seg_slots = 0, n_maps = 1, tiles = 1;
     size_t tsz = 0;                 // doubles per site tensor
@@ -64,8 +65,9 @@ struct Plan {
 
 inline bool make_plan(Plan& p, int L, int chi, int n_dis, int n_samples_max, int ckpt, int prec = 0, int real_j = 0) {
     p.real_j = real_j;
-    if (prec != 0 && prec != 1) return false;
-    p.f32 = prec == 1;
+    if (prec < 0 || prec > 2) return false;
+    p.f32 = prec != 0;
+    p.tf32 = prec == 1;
     if (L < 2 || L > 4096 || chi < 2 || chi > 32 || n_dis < 1 || n_samples_max < 1 || ckpt < 0) return false;
     if (ckpt >= L) ckpt = 0;
     p.L = L; p.chi = chi; p.P = pad_chi(chi); p.W = (L + 31) / 32; p.n_dis = n_dis;
@@ -118,5 +120,5 @@ struct tnmc_ctx {
         return v;
     }
     const int* map(int m) const { return at<int>(plan.off_maps) + (size_t)m * plan.L; }
-    tnmc::EnvRef env() const { tnmc::EnvRef e; e.base = ws + plan.off_env; e.f32 = plan.f32; return e; }
+    tnmc::EnvRef env() const { tnmc::EnvRef e; e.base = ws + plan.off_env; e.f32 = plan.f32; e.lay32 = plan.tf32; return e; }
 };

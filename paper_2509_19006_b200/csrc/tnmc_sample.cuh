@@ -16,6 +16,8 @@
 // and k-tile kt, slot q  <->  bond index 8*(kt/2) + 2q + (kt%2), so the C fragments of one site
 // are, register for register, the A fragments of the next.
 #pragma once
+#include <type_traits>
+
 #include "tnmc_common.cuh"
 
 namespace tnmc {
@@ -65,8 +67,9 @@ __device__ __forceinline__ double quad_sum(double v) {
     return v;
 }
 
-template <int P, bool REALJ>
+template <int P, bool REALJ, bool F32READ>
 __global__ void __launch_bounds__(SAMPLE_THREADS, (P <= 16 ? 2 : 1)) sample_rows_kernel(const SampleArgs args) {
+    typedef typename std::conditional<F32READ, float, double>::type TS;   // storage type of the site tensors (TNMC_F32_STORE: float)
     constexpr int KT = P / 4;        // k tiles
     constexpr int NT = P / 4;        // n tiles (2P / 8)
     constexpr int JT = P / 8;        // 8-wide tiles per spin slice
@@ -86,7 +89,7 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, (P <= 16 ? 2 : 1)) sample_rows
     const int tile = blockIdx.x;
     const double beta = args.beta;
     const double eb = exp(beta), emb = exp(-beta);
-    const double* env_d = reinterpret_cast<const double*>(args.env.base) + (size_t)d * args.env_dis_stride;
+    const TS* env_d = reinterpret_cast<const TS*>(args.env.base) + (size_t)d * args.env_dis_stride;
     double* renv = args.renv + ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * (size_t)L * SAMPLE_CHAINS * P;
 
     // chain handled as M-tile mt, row g of this warp
@@ -128,9 +131,10 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, (P <= 16 ? 2 : 1)) sample_rows
     auto issue_prefetch = [&]() {
         if (pf_r < args.row_hi) {
             const int site = pf_t < L - 1 ? (L - 1 - pf_t) : (pf_t - (L - 1));
-            const double* src = env_d + ((size_t)args.slot_of_row[pf_r] * L + site) * TSZ;
-            double* dst = sT + pf_stage * TSZ;
-            for (int o = tid * 2; o < TSZ; o += SAMPLE_THREADS * 2) cp_async16(dst + o, src + o);
+            const TS* src = env_d + ((size_t)args.slot_of_row[pf_r] * L + site) * TSZ;
+            TS* dst = reinterpret_cast<TS*>(sT) + pf_stage * TSZ;
+            constexpr int V = 16 / (int)sizeof(TS);
+            for (int o = tid * V; o < TSZ; o += SAMPLE_THREADS * V) cp_async16(dst + o, src + o);
             if (++pf_t == steps_per_row) { pf_t = 0; ++pf_r; }
         }
         if (++pf_stage == SAMPLE_STAGES) pf_stage = 0;
@@ -174,7 +178,7 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, (P <= 16 ? 2 : 1)) sample_rows
             cp_async_wait<SAMPLE_STAGES - 2>();
             __syncthreads();
             issue_prefetch();
-            const double* T = sT + cur_stage * TSZ;   // tensor of site col+1
+            const TS* T = reinterpret_cast<const TS*>(sT) + cur_stage * TSZ;   // tensor of site col+1
             if (++cur_stage == SAMPLE_STAGES) cur_stage = 0;
             const int site = col + 1;
             if ((site >> 5) != cur_word) {
@@ -197,7 +201,7 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, (P <= 16 ? 2 : 1)) sample_rows
 #pragma unroll
                 for (int nt = 0; nt < NT; ++nt) {
                     const int a = nt / JT, i = 8 * (nt % JT) + g;
-                    const double b = T[env_off(P, i, a, j)];
+                    const double b = (double)T[env_off(P, i, a, j)];
 #pragma unroll
                     for (int mt = 0; mt < MT; ++mt) dmma884(acc[mt][nt][0], acc[mt][nt][1], vf[mt][kt], b);
                 }
@@ -248,7 +252,7 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, (P <= 16 ? 2 : 1)) sample_rows
             cp_async_wait<SAMPLE_STAGES - 2>();
             __syncthreads();
             issue_prefetch();
-            const double* T = sT + cur_stage * TSZ;   // tensor of site col
+            const TS* T = reinterpret_cast<const TS*>(sT) + cur_stage * TSZ;   // tensor of site col
             if (++cur_stage == SAMPLE_STAGES) cur_stage = 0;
             if ((col >> 5) != cur_word) {
                 cur_word = col >> 5;
@@ -271,7 +275,7 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, (P <= 16 ? 2 : 1)) sample_rows
             for (int kt = 0; kt < KT; ++kt)
 #pragma unroll
                 for (int nt = 0; nt < NT; ++nt) {
-                    const double b = T[(kt * NT + nt) * 32 + lane];
+                    const double b = (double)T[(kt * NT + nt) * 32 + lane];
 #pragma unroll
                     for (int mt = 0; mt < MT; ++mt) dmma884(acc[mt][nt][0], acc[mt][nt][1], vf[mt][kt], b);
                 }

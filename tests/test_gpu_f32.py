@@ -91,3 +91,39 @@ def test_f32_exact_chi_residual(tn):
     acc, n_acc, _, _ = ctx.tnmc_metropolis(E, logq, c["seed"])
     assert (n_acc >= 0.8 * n_s).all()
     assert tn.tnmc_workspace_bytes(64, 32, 10, 8, prec=tn.TNMC_F32_LOGSCALE) < tn.tnmc_workspace_bytes(64, 32, 10, 8)
+
+
+@pytest.mark.parametrize("L,chi,beta,k", [(12, 8, 1.0, 0), (24, 32, 1.0, 0), (32, 16, 2.0, 0), (20, 16, 1.0, 6)])
+def test_f32_store_mode(tn, L, chi, beta, k):
+    """TNMC_F32_STORE: FP32 stack, all arithmetic FP64.  Conditionals stay within ~1e-5 of the FP64 path (the
+    tensors are rounded once per stored row), log Z within 1e-4 of the oracle, q normalised by construction
+    (log q = sum of the logs of the reported conditionals, teacher forcing reproduces it bit for bit)."""
+    n_dis, n_s, seed = 2, 40, 9
+    Jr, Jd = make_couplings(L, n_dis, 900 + L)
+    ctx = _ctx(tn, L, chi, beta, Jr, Jd, n_s, prec=tn.TNMC_F32_STORE, ckpt_stride=k)
+    ref = _ctx(tn, L, chi, beta, Jr, Jd, n_s)
+    logZ = ctx.tnmc_build_envs().cpu().numpy()
+    ref.tnmc_build_envs()
+    probs = torch.zeros((n_dis, n_s, L, L), dtype=torch.float64, device="cuda")
+    bits, logq = ctx.tnmc_sample(n_s, seed, probs=probs)
+    flags = ctx.tnmc_get_flags()
+    assert flags["nonfinite"] == 0 and flags["jacobi_limit"] == 0 and flags["logz_nonpos"] == 0 and flags["rho_zero"] == 0
+    for d in range(n_dis):
+        cache, ls = bmps.build_cache(Jr[d], Jd[d], beta, chi)
+        lz, _ = bmps.log_z(cache[0], ls[0])
+        assert abs(logZ[d] - lz) <= 1e-4 * abs(lz)
+    b2, q2 = ctx.tnmc_sample(n_s, seed, forced_cfg_bits=bits)
+    assert torch.equal(b2, bits) and torch.equal(q2, logq)
+    cfg = unpack(bits.cpu().numpy().view(np.uint32), L)
+    p = probs.cpu().numpy()
+    with np.errstate(divide="ignore"):
+        lq = np.where(cfg == 1, np.log(p), np.log1p(-p)).sum(axis=(2, 3))
+    assert np.abs(lq - logq.cpu().numpy()).max() < 1e-9 * L * L
+    p64 = torch.zeros_like(probs)
+    _, q64 = ref.tnmc_sample(n_s, seed, forced_cfg_bits=bits, probs=p64)
+    assert (probs - p64).abs().mean().item() < 1e-5
+    E = ctx.tnmc_energy(bits)
+    acc, n_acc, _, _ = ctx.tnmc_metropolis(E, logq, seed)
+    acc64, n_acc64, _, _ = ref.tnmc_metropolis(E, q64, seed)
+    assert abs(int(n_acc.sum()) - int(n_acc64.sum())) <= 0.05 * n_dis * n_s
+    assert tn.tnmc_workspace_bytes(64, 32, 10, 8, prec=tn.TNMC_F32_STORE) < tn.tnmc_workspace_bytes(64, 32, 10, 8)
