@@ -48,8 +48,10 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="C2", choices=sorted(WORKLOADS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--prec", default="f64", choices=["f64", "f32"],
-                    help="f64: the parity path; f32: TNMC_F32_LOGSCALE (FP32 stack, TF32 tensor-core sampler, FP64 compression)")
+    ap.add_argument("--prec", default="f64", choices=["f64", "f32", "f32s"],
+                    help="f64: the parity path; f32: TNMC_F32_LOGSCALE (FP32 stack, TF32 tensor-core sampler, FP64 compression); "
+                         "f32s: TNMC_F32_STORE (FP32 stack, all arithmetic FP64)")
+    ap.add_argument("--chunk", type=int, default=0, help="disorders per chunk (overrides the workload's; 0 = its default)")
     ap.add_argument("--couplings", default="pmj", choices=["pmj", "gaussian"],
                     help="pmj: +-J (the BASELINE configs); gaussian: J ~ N(0,1) through tnmc_create_real (no e2e / cpu_baseline leg)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -207,6 +209,8 @@ def main_ours(args):
     c = workload(args.workload)
     L, chi, n_dis, n_s, ckpt = c["L"], c["chi"], c["n_dis"], c["n_samples"], c["ckpt"]
     n_dis_total = n_dis                                   # per rank
+    if args.chunk:
+        c["chunk"] = args.chunk
     if c.get("chunk"):
         n_dis = min(c["chunk"], n_dis_total)              # buffers and contexts are sized for one chunk
     chunks = [(c0, min(n_dis, n_dis_total - c0)) for c0 in range(0, n_dis_total, n_dis)]
@@ -221,7 +225,7 @@ def main_ours(args):
     Jr_np, Jd_np = gen(L, n_dis_total, c["inst_seed"], first_disorder=first)
     Jr_h, Jd_h = torch.from_numpy(Jr_np).pin_memory(), torch.from_numpy(Jd_np).pin_memory()
     Jr, Jd = Jr_h.to(dev), Jd_h.to(dev)
-    prec = tnmc.TNMC_F32_LOGSCALE if args.prec == "f32" else tnmc.TNMC_F64
+    prec = {"f64": tnmc.TNMC_F64, "f32": tnmc.TNMC_F32_LOGSCALE, "f32s": tnmc.TNMC_F32_STORE}[args.prec]
     need = tnmc.tnmc_workspace_bytes(L, chi, n_dis, n_s, prec=prec, ckpt_stride=ckpt)
     if real_j:
         need = int(tnmc.lib.tnmc_workspace_bytes_real(L, chi, n_dis, n_s, prec, ckpt))
@@ -362,7 +366,7 @@ def main_ours(args):
             pass
         hbm_peak = peaks.get("hbm_gbs", 6650.0)
         samp_flops = nb * model.sample_flops_per_chain_site(P) * n_dis_total * n_s * L * L
-        w_env = 4 if args.prec == "f32" else 8
+        w_env = 8 if args.prec == "f64" else 4
         samp_bytes = nb * model.sample_bytes_per_chain_site(P, w=w_env) * n_dis_total * n_s * L * L
         if ckpt:
             # checkpoint mode: tnmc_sample recomputes every segment with build_rows_kernel before sampling it, so the
@@ -399,7 +403,7 @@ def main_ours(args):
                    "sample": f"{n_d} disorders x {n_so} samples x {len(betas)} betas of {args.workload} (whole path)"}
         line = {"metric": "accepted samples/s", "value": value, "unit": "samples/s", "n_gpus": world, "steps": args.steps,
                 "warmup": n_warm, "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak",
-                "vs_baseline": None, "dtype": "f64" if args.prec == "f64" else "f64 compression + tf32 sampling (fp32 stack)", "data": "synthetic",
+                "vs_baseline": None, "dtype": {"f64": "f64", "f32": "f64 compression + tf32 sampling (fp32 stack)", "f32s": "f64 arithmetic on an fp32 stack"}[args.prec], "data": "synthetic",
                 "config": {"workload": args.workload, "couplings": args.couplings, "note": c["note"], "L": L, "chi": chi, "betas": betas, "n_dis_per_gpu": n_dis_total, "disorder_chunks": len(chunks),
                            "n_samples": n_s, "ckpt_stride": ckpt, "parallelism": f"dp{world} (disorders sharded, no collective)",
                            "l2": "flushed (256 MiB memset) between timed steps; env stack > L2",
