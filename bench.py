@@ -36,9 +36,10 @@ WORKLOADS = {
     # the full configs[3] / configs[4]: disorder chunks of the same calls, one after the other in the same workspace
     "C4": ("C4", None, None, 23, "configs[3] 512x512 chi=32, 500 disorders x 200 samples in 2 chunks of 250 disorders, checkpoint stride 23", 250),
     "C5": ("C5", None, None, 32, "configs[4] 1024x1024 chi=32, 1000 disorders x 1000 samples in 10 chunks of 100 disorders (152 GB of HBM per chunk), checkpoint stride 32", 100),
+    "C5c": ("C5", 100, 1000, 32, "configs[4] 1024x1024 chi=32: ONE of the ten 100-disorder chunks of C5 (100 disorders x 1000 samples, 152 GB of HBM), checkpoint stride 32"),
     "C5p": ("C5p", 500, 400, 32, "the paper headline setting (1024x1024, chi=8, PAPER.md:286) in FP64: slice of 500 disorders x 400 samples (one fifth of its 10^6 proposals), checkpoint stride 32"),
 }
-SLICES = ("C4s", "C5s", "C5p", "C4", "C5")   # steps of minutes to hours: --warmup is taken as given (0 allowed; said in config)
+SLICES = ("C4s", "C5s", "C5c", "C5p", "C4", "C5")   # steps of minutes to hours: --warmup is taken as given (0 allowed; said in config)
 
 
 def parse():
