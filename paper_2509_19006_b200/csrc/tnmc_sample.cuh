@@ -68,7 +68,7 @@ __device__ __forceinline__ double quad_sum(double v) {
 }
 
 template <int P, bool REALJ, bool F32READ>
-__global__ void __launch_bounds__(SAMPLE_THREADS, (P <= 16 ? 2 : 1)) sample_rows_kernel(const SampleArgs args) {
+__global__ void __launch_bounds__(SAMPLE_THREADS, 2) sample_rows_kernel(const SampleArgs args) {
     typedef typename std::conditional<F32READ, float, double>::type TS;   // storage type of the site tensors (TNMC_F32_STORE: float)
     constexpr int KT = P / 4;        // k tiles
     constexpr int NT = P / 4;        // n tiles (2P / 8)
