@@ -25,7 +25,7 @@ __device__ __forceinline__ void raise_flag(unsigned long long* flags, int which)
 // mma.sync.m8n8k4.f64 as the B operand with one conflict-free 8-byte shared-memory load per lane:
 //   k-tile kt holds the four left-bond indices i = 8*(kt/2) + 2*q + (kt%2), q = 0..3
 //   n-tile nt holds the eight columns (a, j) with a = nt / (P/8), j = 8*(nt % (P/8)) + g, g = 0..7
-//   element offset = ((kt * NT + nt) * 32 + g*4 + q),  NT = P/4,  lane = g*4 + q.
+//   element offset = ((kt * NT + nt) * 32 + ((g*4 + q) ^ 4*(kt%2))),  NT = P/4,  lane = g*4 + q.
 // The odd/even split of i over two k-tiles is what lets the accumulator fragment of one site
 // (lane q holds columns 2q, 2q+1 of each n-tile) be used, unshuffled, as the A fragment of the
 // next site.
@@ -37,7 +37,10 @@ __host__ __device__ __forceinline__ int env_off(int P, int i, int a, int j) {
     const int q = (i & 7) >> 1;
     const int nt = a * (P >> 3) + (j >> 3);
     const int g = j & 7;
-    return ((kt * (P >> 2) + nt) * 32 + g * 4 + q);
+    // odd k-tiles are stored with bit 2 of the in-tile index flipped: a permutation inside the tile for the left
+    // sweep (still one conflict-free 8-byte load per lane), and it puts the two k-tile parities that the right
+    // sweep's transposed read touches in one half-warp on disjoint banks
+    return ((kt * (P >> 2) + nt) * 32 + ((g * 4 + q) ^ ((kt & 1) << 2)));
 }
 
 // FP32 storage (TNMC_F32_LOGSCALE) uses the fragment order of mma.sync.m16n8k8.tf32 instead: k-tile kt

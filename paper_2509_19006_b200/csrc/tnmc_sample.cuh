@@ -275,7 +275,7 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, 2) sample_rows_kernel(const Sa
             for (int kt = 0; kt < KT; ++kt)
 #pragma unroll
                 for (int nt = 0; nt < NT; ++nt) {
-                    const double b = (double)T[(kt * NT + nt) * 32 + lane];
+                    const double b = (double)T[(kt * NT + nt) * 32 + (lane ^ ((kt & 1) << 2))];
 #pragma unroll
                     for (int mt = 0; mt < MT; ++mt) dmma884(acc[mt][nt][0], acc[mt][nt][1], vf[mt][kt], b);
                 }
