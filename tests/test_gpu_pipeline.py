@@ -187,3 +187,26 @@ def test_config_c2_subset(tn, beta):
         assert np.abs(p_gpu[ok] - o_probs[ok]).max() < tol_p
         assert np.abs(logq[d, :n_chk].cpu().numpy()[ok] - o_logq[ok]).max() < max(1e-9 * np.abs(o_logq).max(), nf.FLOOR_FACTOR * fl_q)
         assert (E[d, :n_chk][ok] == exact.energy(o_cfg[ok], Jr[d], Jd[d])).all()
+
+
+@pytest.mark.parametrize("L,chi,n_dis,n_s", [(2, 2, 1, 1), (3, 32, 2, 2), (5, 32, 1, 129), (2, 32, 3, 1)])
+def test_degenerate_sizes(tn, L, chi, n_dis, n_s):
+    """smallest lattice, one sample, chi far above the exact bound (the padded-bond code paths with tiny bonds),
+    one chain more than a tile: exact chi, so log q = -beta E - log Z and log Z = brute force."""
+    beta, seed = 0.9, 3
+    Jr, Jd = make_couplings(L, n_dis, 70 + L)
+    ctx = _ctx(tn, L, chi, beta, Jr, Jd, n_s)
+    logZ = ctx.tnmc_build_envs()
+    bits, logq = ctx.tnmc_sample(n_s, seed)
+    E = ctx.tnmc_energy(bits)
+    acc, n_acc, _, _ = ctx.tnmc_metropolis(E, logq, seed)
+    flags = ctx.tnmc_get_flags()
+    assert flags["nonfinite"] == 0 and flags["jacobi_limit"] == 0 and flags["rho_zero"] == 0 and flags["logz_nonpos"] == 0
+    for d in range(n_dis):
+        _, _, lz, _ = exact.brute_force(Jr[d], Jd[d], beta)
+        assert abs(logZ[d].item() - lz) < 1e-10 * abs(lz)
+    assert (logq + beta * E.double() + logZ[:, None]).abs().max().item() < 1e-9
+    assert (n_acc == n_s - 1).all() and (acc[:, 0] == 1).all()
+    cfg = unpack(_u32(bits), L)
+    for d in range(n_dis):
+        assert (E[d].cpu().numpy() == exact.energy(cfg[d], Jr[d], Jd[d])).all()
