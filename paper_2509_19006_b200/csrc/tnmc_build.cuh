@@ -262,14 +262,14 @@ __global__ void __launch_bounds__(BuildCfg<P>::NT, BuildCfg<P>::CTAS_PER_SM) bui
             int* spst = sperm;                       // step at which each column was the pivot
             const double fro2 = householder_qrcp2<MAXK>(sX, LDX, q, nc, sCn, sWk, spst, sNr);
             const int nrow = *sNr;                   // rows of R kept (even)
-            for (int t = tid; t < nrow * nc; t += NT) {
-                const int j = t % nc, i = t / nc;
-                sMj[(size_t)i * LDM + j] = i <= spst[j] ? sX[i + (size_t)j * LDX] : 0.0;
+            for (int t = tid; t < nrow * D; t += NT) {      // rows zero-padded to D columns for the Jacobi
+                const int j = t % D, i = t / D;
+                sMj[(size_t)i * LDM + j] = (j < nc && i <= spst[j]) ? sX[i + (size_t)j * LDX] : 0.0;
             }
             __syncthreads();
             const double thr2 = fro2 * 1e-30;      // sigma <= 1e-15 |M|_F: below the numerical rank
             PROF(4);
-            const int nsw = nrow >= 2 ? jacobi_rows2<(D + 2 * Cfg::LPP - 1) / (2 * Cfg::LPP), Cfg::LPP>(sMj, LDM, nrow, nc, fro2, thr2, args.flags) : 0;
+            const int nsw = nrow >= 2 ? jacobi_rows2<(D + 2 * Cfg::LPP - 1) / (2 * Cfg::LPP), Cfg::LPP>(sMj, LDM, nrow, fro2, thr2, args.flags) : 0;
             PROF(5);
             PROF_ADD(8, nsw); PROF_ADD(9, 1);
             (void)nsw;

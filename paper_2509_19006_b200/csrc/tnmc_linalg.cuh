@@ -321,10 +321,11 @@ __device__ double householder_qrcp2(double* X, int ld, int m, int n, double* cn,
 // updated after a rotation and nothing is refreshed per sweep; and the rotation comes from two FP64
 // rsqrt with no division and no FP32 detour:
 //   d = b - a, h = sqrt(d^2 + 4 g^2), u = |d| + h, w = 1 / sqrt(u^2 + 4 g^2), cos = u w, sin = sign(d) 2 g w.
+// The caller zero-pads every row to the full 2 LPP NK columns (rotations keep zeros zero).
 // All n rows take part (n even); rows at or below thr2 are left alone.  LPP lanes per row pair (a power of
 // two <= 8), NK = ceil(max nc / (2 LPP)) column pairs per lane.  Returns the sweeps done.
 template <int NK, int LPP>
-__device__ int jacobi_rows2(double* M, int ld, int n, int nc, double fro2, double thr2, unsigned long long* flags) {
+__device__ int jacobi_rows2(double* M, int ld, int n, double fro2, double thr2, unsigned long long* flags) {
     const int grp = threadIdx.x / LPP, t8 = threadIdx.x % LPP;
     const int npairs = n >> 1;
     const unsigned gmask = ((1u << LPP) - 1u) << ((threadIdx.x & 31) & ~(LPP - 1));
@@ -348,12 +349,10 @@ __device__ int jacobi_rows2(double* M, int ld, int n, int nc, double fro2, doubl
                 double* y = M + (size_t)r2 * ld;
                 double2 xv[NK], yv[NK];
 #pragma unroll
-                for (int k = 0; k < NK; ++k) {
+                for (int k = 0; k < NK; ++k) {      // rows are zero-padded to the full 2 LPP NK columns: no bounds checks
                     const int c = c0 + 2 * LPP * k;
-                    if (c < nc) {
-                        xv[k] = *reinterpret_cast<const double2*>(x + c);
-                        yv[k] = *reinterpret_cast<const double2*>(y + c);
-                    } else { xv[k] = make_double2(0.0, 0.0); yv[k] = make_double2(0.0, 0.0); }
+                    xv[k] = *reinterpret_cast<const double2*>(x + c);
+                    yv[k] = *reinterpret_cast<const double2*>(y + c);
                 }
                 double a = 0.0, b = 0.0, g = 0.0, a1 = 0.0, b1 = 0.0, g1 = 0.0;
 #pragma unroll
@@ -384,13 +383,11 @@ __device__ int jacobi_rows2(double* M, int ld, int n, int nc, double fro2, doubl
 #pragma unroll
                     for (int k = 0; k < NK; ++k) {
                         const int c = c0 + 2 * LPP * k;
-                        if (c < nc) {
-                            double2 xn, yn;
-                            xn.x = fma(cs, xv[k].x, -sn * yv[k].x);  yn.x = fma(sn, xv[k].x, cs * yv[k].x);
-                            xn.y = fma(cs, xv[k].y, -sn * yv[k].y);  yn.y = fma(sn, xv[k].y, cs * yv[k].y);
-                            *reinterpret_cast<double2*>(x + c) = xn;
-                            *reinterpret_cast<double2*>(y + c) = yn;
-                        }
+                        double2 xn, yn;
+                        xn.x = fma(cs, xv[k].x, -sn * yv[k].x);  yn.x = fma(sn, xv[k].x, cs * yv[k].x);
+                        xn.y = fma(cs, xv[k].y, -sn * yv[k].y);  yn.y = fma(sn, xv[k].y, cs * yv[k].y);
+                        *reinterpret_cast<double2*>(x + c) = xn;
+                        *reinterpret_cast<double2*>(y + c) = yn;
                     }
                 }
             }
