@@ -91,6 +91,76 @@ __device__ __forceinline__ double quad_dot_update(const double* __restrict__ v, 
     return w;
 }
 
+// The number of live rows shrinks as the factorization proceeds: pick the smallest unrolled depth (a quarter,
+// a half, three quarters or all of MAXK rows per lane) that covers rows i0 .. m-1.  The choice is uniform over the
+// CTA (m and i0 are), so no divergence; it removes on average half of the predicated loads and FMAs of a sweep.
+template <int MAXK>
+__device__ __forceinline__ double quad_dot_update_n(const double* __restrict__ v, double* __restrict__ col,
+                                                    int i0, int m, int rg, unsigned qmask, double tau, double head,
+                                                    double& below2) {
+    const int rows = m - i0;
+    if (MAXK >= 4) {
+        if (rows <= MAXK) return quad_dot_update<(MAXK + 3) / 4>(v, col, i0, m, rg, qmask, tau, head, below2);
+        if (rows <= 2 * MAXK) return quad_dot_update<MAXK / 2>(v, col, i0, m, rg, qmask, tau, head, below2);
+        if (rows <= 3 * MAXK) return quad_dot_update<(3 * MAXK) / 4>(v, col, i0, m, rg, qmask, tau, head, below2);
+    }
+    return quad_dot_update<MAXK>(v, col, i0, m, rg, qmask, tau, head, below2);
+}
+
+// The same update with the UNSCALED pivot column pc (the reflector vector is pc * scale below row j) and the scalars
+// (tau, scale) applied on the fly: w = tau (cj + scale * sum_i pc_i col_i), col_i -= w scale pc_i, row j -> cj - w.
+// Returns the squared norm of the updated rows below j (summed over the quad).
+template <int K>
+__device__ __forceinline__ double quad_pivot_update(const double* __restrict__ pc, double* __restrict__ col,
+                                                    int j, int m, int rg, unsigned qmask, double tau, double scale) {
+    double x[K], vv[K];
+    double w0 = 0.0, w1 = 0.0;
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        const int i = j + 1 + rg + 4 * k;
+        const bool in = i < m;
+        x[k] = in ? col[i] : 0.0;
+        vv[k] = in ? pc[i] : 0.0;
+    }
+    const double cj = col[j];
+#pragma unroll
+    for (int k = 0; k < K; k += 2) {
+        w0 = fma(vv[k], x[k], w0);
+        if (k + 1 < K) w1 = fma(vv[k + 1], x[k + 1], w1);
+    }
+    double dot = w0 + w1;
+    dot += __shfl_xor_sync(qmask, dot, 1);
+    dot += __shfl_xor_sync(qmask, dot, 2);
+    const double w = tau * fma(scale, dot, cj);
+    const double ws = w * scale;
+    double s0 = 0.0, s1 = 0.0;
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        const int i = j + 1 + rg + 4 * k;
+        if (i < m) {
+            const double nv = fma(-ws, vv[k], x[k]);
+            col[i] = nv;
+            if (k & 1) s1 = fma(nv, nv, s1); else s0 = fma(nv, nv, s0);
+        }
+    }
+    double below2 = s0 + s1;
+    below2 += __shfl_xor_sync(qmask, below2, 1);
+    below2 += __shfl_xor_sync(qmask, below2, 2);
+    if (rg == 0) col[j] = cj - w;
+    return below2;
+}
+template <int MAXK>
+__device__ __forceinline__ double quad_pivot_update_n(const double* __restrict__ pc, double* __restrict__ col,
+                                                      int j, int m, int rg, unsigned qmask, double tau, double scale) {
+    const int rows = m - j - 1;
+    if (MAXK >= 4) {
+        if (rows <= MAXK) return quad_pivot_update<(MAXK + 3) / 4>(pc, col, j, m, rg, qmask, tau, scale);
+        if (rows <= 2 * MAXK) return quad_pivot_update<MAXK / 2>(pc, col, j, m, rg, qmask, tau, scale);
+        if (rows <= 3 * MAXK) return quad_pivot_update<(3 * MAXK) / 4>(pc, col, j, m, rg, qmask, tau, scale);
+    }
+    return quad_pivot_update<MAXK>(pc, col, j, m, rg, qmask, tau, scale);
+}
+
 // Reflector from alpha = x_j and nrm2 = sum_{i >= j} x_i^2 (the diagonal entry included, so no
 // cancellation): beta = -sign(alpha) sqrt(nrm2), tau = (beta - alpha) / beta, v_i = x_i / (alpha - beta).
 __device__ __forceinline__ void reflector_from_norm(double alpha, double nrm2, double& beta, double& tau, double& scale) {
@@ -143,7 +213,7 @@ __device__ void householder_qr_g(double* X, int ld, int m, int n, double* tau, i
         if (jj < n) {
             double* col = X + (size_t)jj * ld;
             double below2;
-            const double w = quad_dot_update<MAXK>(colj, col, j + 1, m, rg, qmask, t, col[j], below2);
+            const double w = quad_dot_update_n<MAXK>(colj, col, j + 1, m, rg, qmask, t, col[j], below2);
             if (rg == 0) col[j] -= w;
             if (colidx == 0 && j + 1 < kk) {       // build reflector j+1 from the updated column
                 below2 += __shfl_xor_sync(qmask, below2, 1);
@@ -174,7 +244,7 @@ __device__ void householder_apply_g(const double* V, int ldv, const double* tau,
         double* col = B + (size_t)colidx * ldb;
         for (int j = kk - 1; j >= 0; --j) {
             double below2;
-            const double w = quad_dot_update<MAXK>(V + (size_t)j * ldv, col, j + 1, m, rg, qmask, tau[j], col[j], below2);
+            const double w = quad_dot_update_n<MAXK>(V + (size_t)j * ldv, col, j + 1, m, rg, qmask, tau[j], col[j], below2);
             __syncwarp(qmask);
             if (rg == 0) col[j] -= w;
             __syncwarp(qmask);
@@ -262,42 +332,9 @@ __device__ double householder_qrcp2(double* X, int ld, int m, int n, double* cn,
         const double* pc = X + (size_t)bi * ld;
         double bet, tau, scale;
         if (active && cq != bi) {
-            // dot product with the unscaled pivot column, beside the scalar chain
-            double x[MAXK], vv[MAXK];
-            double w0 = 0.0, w1 = 0.0;
-#pragma unroll
-            for (int k = 0; k < MAXK; ++k) {
-                const int i = j + 1 + rg + 4 * k;
-                const bool in = i < m;
-                x[k] = in ? col[i] : 0.0;
-                vv[k] = in ? pc[i] : 0.0;
-            }
-            const double cj = col[j];
+            // dot product with the unscaled pivot column; the scalars are folded in on the fly
             reflector_from_norm(pc[j], best, bet, tau, scale);
-#pragma unroll
-            for (int k = 0; k < MAXK; k += 2) {
-                w0 = fma(vv[k], x[k], w0);
-                if (k + 1 < MAXK) w1 = fma(vv[k + 1], x[k + 1], w1);
-            }
-            double dot = w0 + w1;
-            dot += __shfl_xor_sync(qmask, dot, 1);
-            dot += __shfl_xor_sync(qmask, dot, 2);
-            const double w = tau * fma(scale, dot, cj);
-            const double ws = w * scale;
-            double s0 = 0.0, s1 = 0.0;
-#pragma unroll
-            for (int k = 0; k < MAXK; ++k) {
-                const int i = j + 1 + rg + 4 * k;
-                if (i < m) {
-                    const double nv = fma(-ws, vv[k], x[k]);
-                    col[i] = nv;
-                    if (k & 1) s1 = fma(nv, nv, s1); else s0 = fma(nv, nv, s0);
-                }
-            }
-            double below2 = s0 + s1;
-            below2 += __shfl_xor_sync(qmask, below2, 1);
-            below2 += __shfl_xor_sync(qmask, below2, 2);
-            if (rg == 0) col[j] = cj - w;
+            const double below2 = quad_pivot_update_n<MAXK>(pc, col, j, m, rg, qmask, tau, scale);
             myn = below2;
         } else if (active) {   // this quad owns the pivot: its column is final (row j becomes beta, written after the barrier)
             reflector_from_norm(pc[j], best, bet, tau, scale);
