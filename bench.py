@@ -377,7 +377,10 @@ def main_ours(args):
         dominant = "build_rows_kernel" if (ckpt or phases["build"] >= phases["sample"]) else "sample_rows_kernel"
         traffic = None                                       # DRAM bytes per launch from the committed ncu capture (profiles/)
         try:
-            traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(args.workload, {}).get(dominant)
+            for ln in open(os.path.join(ROOT, "profiles", "traffic.csv")).read().splitlines()[1:]:
+                w_, k_, b_ = ln.split(",")[:3]
+                if w_ == args.workload and k_ == dominant:
+                    traffic = int(b_)
         except Exception:
             pass
         if dominant == "build_rows_kernel":
