@@ -321,11 +321,13 @@ __device__ double householder_qrcp2(double* X, int ld, int m, int n, double* cn,
     int j = 0;
     for (; j < kk; ++j) {
         const int buf = j & 1;
-        unsigned mh = wk[buf * 24], ml = wk[buf * 24 + 8], mc = wk[buf * 24 + 16];
-        for (int w = 1; w < nw; ++w) {
-            const unsigned h2 = wk[buf * 24 + w], l2 = wk[buf * 24 + 8 + w], c2 = wk[buf * 24 + 16 + w];
-            if (h2 > mh || (h2 == mh && (l2 > ml || (l2 == ml && c2 < mc)))) { mh = h2; ml = l2; mc = c2; }
-        }
+        // second level of the same reduction: lane w < nw takes warp w's candidate, three redux over the warp
+        const unsigned ch = lane < nw ? wk[buf * 24 + lane] : 0u;
+        const unsigned cl = lane < nw ? wk[buf * 24 + 8 + lane] : 0u;
+        const unsigned cc = lane < nw ? wk[buf * 24 + 16 + lane] : 0xffffu;
+        const unsigned mh = __reduce_max_sync(0xffffffffu, ch);
+        const unsigned ml = __reduce_max_sync(0xffffffffu, ch == mh ? cl : 0u);
+        const unsigned mc = __reduce_min_sync(0xffffffffu, (ch == mh && cl == ml) ? cc : 0xffffu);
         const int bi = mh != 0u ? (int)mc : 0;
         const double best = mh != 0u ? __hiloint2double((int)(mh - 1u), (int)ml) : 0.0;
         if ((j & 1) == 0 && !(best * (double)(n - j) > thr2)) break;
