@@ -3,7 +3,7 @@
 paper's Fig. 3), on seeded synthetic +-J instances.
 
     python pacc_sweep.py [--Ls 8,16,...] [--chis 8,16] [--betas 0.66,1.0,1.5] [--n-dis 32] [--n-samples 256]
-                         [--prec f64|f32] [--out gpurun_out/pacc.jsonl]
+                         [--prec f64|f32|f32s] [--out gpurun_out/pacc.jsonl]
 
 One JSON line per (L, chi, beta): P_acc = accepted / (n_dis (n_s - 1)) (reading G15 of DESIGN.md), the mean of
 min(1, ratio), seconds per phase.  Everything runs through the C ABI binding; nothing here touches oracle/."""
@@ -26,7 +26,7 @@ def main():
     ap.add_argument("--betas", default="0.66,1.0,1.5")
     ap.add_argument("--n-dis", type=int, default=32)
     ap.add_argument("--n-samples", type=int, default=256)
-    ap.add_argument("--prec", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--prec", default="f64", choices=["f64", "f32", "f32s"])
     ap.add_argument("--inst-seed", type=int, default=3003)
     ap.add_argument("--seed", type=int, default=4004)
     ap.add_argument("--out", default=None)
@@ -36,7 +36,7 @@ def main():
     if not torch.cuda.is_available():
         raise SystemExit("pacc_sweep.py needs a CUDA device (no CPU fallback)")
     dev = torch.device("cuda:0")
-    prec = tnmc.TNMC_F32_LOGSCALE if a.prec == "f32" else tnmc.TNMC_F64
+    prec = {"f64": tnmc.TNMC_F64, "f32": tnmc.TNMC_F32_LOGSCALE, "f32s": tnmc.TNMC_F32_STORE}[a.prec]
     out = open(a.out, "a") if a.out else None
     for L in [int(x) for x in a.Ls.split(",")]:
         n_dis = a.n_dis
@@ -46,7 +46,7 @@ def main():
         for chi in [int(x) for x in a.chis.split(",")]:
             # full stack while it fits comfortably, else two-level checkpoints with stride ~ sqrt(L)
             P = 8 if chi <= 8 else (16 if chi <= 16 else 32)
-            full_bytes = n_dis * L * L * 2 * P * P * (4 if a.prec == "f32" else 8)
+            full_bytes = n_dis * L * L * 2 * P * P * (8 if a.prec == "f64" else 4)
             ckpt = 0 if full_bytes < 60e9 else max(2, int(round(L ** 0.5)))
             for beta in [float(x) for x in a.betas.split(",")]:
                 ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
