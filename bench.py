@@ -49,8 +49,8 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="C2", choices=sorted(WORKLOADS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--prec", default="f64", choices=["f64", "f32", "f32s"],
-                    help="f64: the parity path; f32: TNMC_F32_LOGSCALE (FP32 stack, TF32 tensor-core sampler, FP64 compression); "
+    ap.add_argument("--prec", default="f64", choices=["f64", "f32", "f32s", "tf32"],
+                    help="f64: the parity path; f32: TNMC_F32_LOGSCALE (FP32 stack, 3xTF32 tensor-core sampler, FP64 compression); tf32: TNMC_TF32_FAST (plain TF32 products); "
                          "f32s: TNMC_F32_STORE (FP32 stack, all arithmetic FP64)")
     ap.add_argument("--chunk", type=int, default=0, help="disorders per chunk (overrides the workload's; 0 = its default)")
     ap.add_argument("--couplings", default="pmj", choices=["pmj", "gaussian"],
@@ -226,7 +226,7 @@ def main_ours(args):
     Jr_np, Jd_np = gen(L, n_dis_total, c["inst_seed"], first_disorder=first)
     Jr_h, Jd_h = torch.from_numpy(Jr_np).pin_memory(), torch.from_numpy(Jd_np).pin_memory()
     Jr, Jd = Jr_h.to(dev), Jd_h.to(dev)
-    prec = {"f64": tnmc.TNMC_F64, "f32": tnmc.TNMC_F32_LOGSCALE, "f32s": tnmc.TNMC_F32_STORE}[args.prec]
+    prec = {"f64": tnmc.TNMC_F64, "f32": tnmc.TNMC_F32_LOGSCALE, "f32s": tnmc.TNMC_F32_STORE, "tf32": tnmc.TNMC_TF32_FAST}[args.prec]
     need = tnmc.tnmc_workspace_bytes(L, chi, n_dis, n_s, prec=prec, ckpt_stride=ckpt)
     if real_j:
         need = int(tnmc.lib.tnmc_workspace_bytes_real(L, chi, n_dis, n_s, prec, ckpt))
@@ -407,7 +407,7 @@ def main_ours(args):
                    "sample": f"{n_d} disorders x {n_so} samples x {len(betas)} betas of {args.workload} (whole path)"}
         line = {"metric": "accepted samples/s", "value": value, "unit": "samples/s", "n_gpus": world, "steps": args.steps,
                 "warmup": n_warm, "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak",
-                "vs_baseline": None, "dtype": {"f64": "f64", "f32": "f64 compression + tf32 sampling (fp32 stack)", "f32s": "f64 arithmetic on an fp32 stack"}[args.prec], "data": "synthetic",
+                "vs_baseline": None, "dtype": {"f64": "f64", "f32": "f64 compression + 3xtf32 sampling (fp32 stack)", "f32s": "f64 arithmetic on an fp32 stack", "tf32": "f64 compression + tf32 sampling (fp32 stack)"}[args.prec], "data": "synthetic",
                 "config": {"workload": args.workload, "couplings": args.couplings, "note": c["note"], "L": L, "chi": chi, "betas": betas, "n_dis_per_gpu": n_dis_total, "disorder_chunks": len(chunks),
                            "n_samples": n_s, "ckpt_stride": ckpt, "parallelism": f"dp{world} (disorders sharded, no collective)",
                            "l2": "flushed (256 MiB memset) between timed steps; env stack > L2",

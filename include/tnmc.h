@@ -75,20 +75,25 @@ typedef enum {
                               environment stack stored in FP32 -- every stored row has unit 2-norm and carries
                               its log-scale separately (reading G7), so single precision has no range problem --
                               and sampling contractions on TF32 tensor cores (mma.sync.m16n8k8, FP32 accumulate,
-                              environments normalised per site).  The compression stays FP64 (it has to resolve
+                              environments normalised per site) with 3xTF32 error compensation (each operand
+                              split into its TF32 part and the exact FP32 remainder, three MMAs per product):
+                              FP32-level accuracy, ~1e-6 per conditional.  The compression stays FP64 (it has to resolve
                               sigma_chi / sigma_1 ~ 1e-9).  Conditional probabilities, the draw and log q are
                               evaluated in FP64 from the FP32 weights with p0 = 1 - p1: q is a normalised
                               distribution and log q is the log of the probabilities actually used, so the
                               Metropolis correction stays exact.  log Z agrees with TNMC_F64 to ~1e-7 relative
-                              (north_star reduced-precision tolerance 1e-4); conditionals carry ~1e-3 of TF32
-                              noise, spins are not bit-identical to the FP64 path, the acceptance is lower.
+                              (north_star reduced-precision tolerance 1e-4); spins are not bit-identical to the
+                              FP64 path.
                               TNMC_FLAG_RHO_ZERO is informational in this mode. */
-    TNMC_F32_STORE = 2     /* environment stack stored in FP32 (in the FP64 sampler's fragment order), ALL arithmetic
+    TNMC_F32_STORE = 2,    /* environment stack stored in FP32 (in the FP64 sampler's fragment order), ALL arithmetic
                               FP64: the tensors are rounded to FP32 once when a row is stored, the compression and
                               the FP64 DMMA sampler read them back as doubles.  Half the HBM footprint and stack
                               traffic at conditionals within ~1e-6 of TNMC_F64 and an unchanged acceptance; spins
                               are not bit-identical to TNMC_F64.  q is normalised and log q is the log of the
                               probabilities used, as in every mode. */
+    TNMC_TF32_FAST = 3     /* as TNMC_F32_LOGSCALE with plain TF32 products (one MMA, 10-bit mantissa inputs): the
+                              fastest sampler (HBM-bound), ~1e-3 of noise per conditional, noticeably lower
+                              acceptance on large lattices.  q stays normalised and log q consistent. */
 } tnmc_prec;
 
 /* indices into the array returned by tnmc_get_flags */

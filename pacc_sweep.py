@@ -26,7 +26,7 @@ def main():
     ap.add_argument("--betas", default="0.66,1.0,1.5")
     ap.add_argument("--n-dis", type=int, default=32)
     ap.add_argument("--n-samples", type=int, default=256)
-    ap.add_argument("--prec", default="f64", choices=["f64", "f32", "f32s"])
+    ap.add_argument("--prec", default="f64", choices=["f64", "f32", "f32s", "tf32"])
     ap.add_argument("--inst-seed", type=int, default=3003)
     ap.add_argument("--seed", type=int, default=4004)
     ap.add_argument("--out", default=None)
@@ -36,7 +36,7 @@ def main():
     if not torch.cuda.is_available():
         raise SystemExit("pacc_sweep.py needs a CUDA device (no CPU fallback)")
     dev = torch.device("cuda:0")
-    prec = {"f64": tnmc.TNMC_F64, "f32": tnmc.TNMC_F32_LOGSCALE, "f32s": tnmc.TNMC_F32_STORE}[a.prec]
+    prec = {"f64": tnmc.TNMC_F64, "f32": tnmc.TNMC_F32_LOGSCALE, "f32s": tnmc.TNMC_F32_STORE, "tf32": tnmc.TNMC_TF32_FAST}[a.prec]
     out = open(a.out, "a") if a.out else None
     for L in [int(x) for x in a.Ls.split(",")]:
         n_dis = a.n_dis

@@ -42,7 +42,7 @@ static tnmc_status create_impl(tnmc_ctx** out, int L, int chi, double beta, int 
     const int real_j = Jr_real != nullptr;
     if (!out) return fail(nullptr, TNMC_EINVAL, "tnmc_create: out is NULL");
     *out = nullptr;
-    if (prec != TNMC_F64 && prec != TNMC_F32_LOGSCALE && prec != TNMC_F32_STORE) return fail(nullptr, TNMC_EINVAL, "tnmc_create: unknown precision");
+    if (prec != TNMC_F64 && prec != TNMC_F32_LOGSCALE && prec != TNMC_F32_STORE && prec != TNMC_TF32_FAST) return fail(nullptr, TNMC_EINVAL, "tnmc_create: unknown precision");
     if (!((Jr && Jd) || (Jr_real && Jd_real)) || !workspace) return fail(nullptr, TNMC_EINVAL, "tnmc_create: NULL pointer");
     if (!(beta >= 0.0) || !std::isfinite(beta)) return fail(nullptr, TNMC_EINVAL, "tnmc_create: beta must be finite and >= 0");
     if ((reinterpret_cast<uintptr_t>(workspace) & 255u) != 0) return fail(nullptr, TNMC_EINVAL, "tnmc_create: workspace must be 256-byte aligned");
@@ -155,16 +155,17 @@ static tnmc_status launch_build(tnmc_ctx* ctx, int m, int row_hi, int row_lo, in
     return TNMC_OK;
 }
 
-// MODE: 0 = FP64 stack + FP64 DMMA sampler, 1 = FP32 stack + TF32 sampler, 2 = FP32 stack + FP64 DMMA sampler
+// MODE: 0 = FP64 stack + FP64 DMMA sampler, 1 = FP32 stack + 3xTF32 sampler, 2 = FP32 stack + FP64 DMMA sampler,
+//       3 = FP32 stack + plain TF32 sampler
 template <int P, int MODE, bool REALJ>
 static cudaError_t launch_sample_t(const tnmc_ctx* ctx, const SampleArgs& a, int tiles, int dis_count) {
     const int W = (a.L + 31) / 32;
-    if (MODE == 1) {
+    if (MODE == 1 || MODE == 3) {
         const size_t smem32 = sizeof(float) * SAMPLE_STAGES * 2 * P * P + sizeof(uint32_t) * SAMPLE_CHAINS * W +
                               (REALJ ? sizeof(float) * 2 * a.L : 0);
-        cudaError_t e32 = cudaFuncSetAttribute(sample_rows_tf32_kernel<P, REALJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem32);
+        cudaError_t e32 = cudaFuncSetAttribute(sample_rows_tf32_kernel<P, REALJ, MODE == 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem32);
         if (e32 != cudaSuccess) return e32;
-        sample_rows_tf32_kernel<P, REALJ><<<dim3(tiles, dis_count), SAMPLE_THREADS, smem32, ctx->stream>>>(a);
+        sample_rows_tf32_kernel<P, REALJ, MODE == 1><<<dim3(tiles, dis_count), SAMPLE_THREADS, smem32, ctx->stream>>>(a);
         return cudaPeekAtLastError();
     }
     const size_t smem = sizeof(double) * SAMPLE_STAGES * 2 * P * P + sizeof(uint32_t) * SAMPLE_CHAINS * W +
@@ -247,7 +248,8 @@ extern "C" tnmc_status tnmc_sample_ex(tnmc_ctx* ctx, int dis_begin, int dis_coun
         } else { a.row_lo = 0; a.row_hi = p.L; }
         a.slot_of_row = ctx->map(m);
         cudaError_t e;
-        if (p.tf32) e = p.real_j ? launch_sample_p<1, true>(ctx, a, tiles, dis_count) : launch_sample_p<1, false>(ctx, a, tiles, dis_count);
+        if (p.tf32 && p.x3) e = p.real_j ? launch_sample_p<1, true>(ctx, a, tiles, dis_count) : launch_sample_p<1, false>(ctx, a, tiles, dis_count);
+        else if (p.tf32) e = p.real_j ? launch_sample_p<3, true>(ctx, a, tiles, dis_count) : launch_sample_p<3, false>(ctx, a, tiles, dis_count);
         else if (p.f32) e = p.real_j ? launch_sample_p<2, true>(ctx, a, tiles, dis_count) : launch_sample_p<2, false>(ctx, a, tiles, dis_count);
         else e = p.real_j ? launch_sample_p<0, true>(ctx, a, tiles, dis_count) : launch_sample_p<0, false>(ctx, a, tiles, dis_count);
         if (e != cudaSuccess) return cuda_fail(ctx, e, "sample_rows_kernel");

@@ -24,7 +24,8 @@ inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 struct Plan {
     int L = 0, chi = 0, P = 0, W = 0, n_dis = 0, n_samples_max = 0, ckpt = 0;
     int f32 = 0;                    // environment stack stored in FP32 (TNMC_F32_LOGSCALE, TNMC_F32_STORE)
-    int tf32 = 0;                   // TF32 tensor-core sampler and its fragment order (TNMC_F32_LOGSCALE)
+    int tf32 = 0;                   // TF32 tensor-core sampler and its fragment order (TNMC_F32_LOGSCALE, TNMC_TF32_FAST)
+    int x3 = 0;                     // error-compensated 3xTF32 products (TNMC_F32_LOGSCALE)
     int real_j = 0;                 // real-valued couplings kept as doubles (tnmc_create_real)
     int n_seg = 1, n_slots = 0, n_seg_slots = 0, n_maps = 1, tiles = 1;
     size_t tsz = 0;                 // doubles per site tensor
@@ -65,9 +66,10 @@ struct Plan {
 
 inline bool make_plan(Plan& p, int L, int chi, int n_dis, int n_samples_max, int ckpt, int prec = 0, int real_j = 0) {
     p.real_j = real_j;
-    if (prec < 0 || prec > 2) return false;
+    if (prec < 0 || prec > 3) return false;
     p.f32 = prec != 0;
-    p.tf32 = prec == 1;
+    p.tf32 = prec == 1 || prec == 3;
+    p.x3 = prec == 1;
     if (L < 2 || L > 4096 || chi < 2 || chi > 32 || n_dis < 1 || n_samples_max < 1 || ckpt < 0) return false;
     if (ckpt >= L) ckpt = 0;
     p.L = L; p.chi = chi; p.P = pad_chi(chi); p.W = (L + 31) / 32; p.n_dis = n_dis;

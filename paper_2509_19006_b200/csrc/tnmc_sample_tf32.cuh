@@ -27,13 +27,32 @@ __device__ __forceinline__ void mma16808_tf32(float& c0, float& c1, float& c2, f
                    "r"(__float_as_uint(b0)), "r"(__float_as_uint(b1)));
 }
 
+// Error-compensated product (3xTF32): x = hi + lo with hi the TF32 part (top 19 bits) and lo = x - hi exact in
+// FP32; a b ~ a_lo b_hi + a_hi b_lo + a_hi b_hi (small terms first), three MMAs, FP32-level accuracy (~1e-6)
+// instead of TF32's ~5e-4 per product.
+__device__ __forceinline__ float tf32_hi(float x) { return __uint_as_float(__float_as_uint(x) & 0xffffe000u); }
+
+template <bool X3>
+__device__ __forceinline__ void mma_tf32_x(float& c0, float& c1, float& c2, float& c3,
+                                           float a0, float a1, float a2, float a3, float b0, float b1) {
+    if (X3) {
+        const float a0h = tf32_hi(a0), a1h = tf32_hi(a1), a2h = tf32_hi(a2), a3h = tf32_hi(a3);
+        const float b0h = tf32_hi(b0), b1h = tf32_hi(b1);
+        mma16808_tf32(c0, c1, c2, c3, a0 - a0h, a1 - a1h, a2 - a2h, a3 - a3h, b0h, b1h);
+        mma16808_tf32(c0, c1, c2, c3, a0h, a1h, a2h, a3h, b0 - b0h, b1 - b1h);
+        mma16808_tf32(c0, c1, c2, c3, a0h, a1h, a2h, a3h, b0h, b1h);
+    } else {
+        mma16808_tf32(c0, c1, c2, c3, a0, a1, a2, a3, b0, b1);
+    }
+}
+
 __device__ __forceinline__ float quad_sumf(float v) {
     v += __shfl_xor_sync(0xffffffffu, v, 1);
     v += __shfl_xor_sync(0xffffffffu, v, 2);
     return v;
 }
 
-template <int P, bool REALJ>
+template <int P, bool REALJ, bool X3>
 __global__ void __launch_bounds__(SAMPLE_THREADS, 2) sample_rows_tf32_kernel(const SampleArgs args) {
     constexpr int KT8 = P / 8;       // k tiles (8 bond indices each)
     constexpr int NT = P / 4;        // n tiles (2P / 8)
@@ -158,7 +177,7 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, 2) sample_rows_tf32_kernel(con
                     const int a = nt / JT, it = nt % JT;
                     const int off = (it * NT + a * JT + kt) * 64 + 8 * q + g;   // env_off32(P, 8 it + g, a, 8 kt + 2q); the odd column is 32 words on
                     const float b0 = T[off], b1 = T[off + 32];
-                    mma16808_tf32(acc[0][nt][0], acc[0][nt][1], acc[1][nt][0], acc[1][nt][1],
+                    mma_tf32_x<X3>(acc[0][nt][0], acc[0][nt][1], acc[1][nt][0], acc[1][nt][1],
                                   vf[0][2 * kt], vf[1][2 * kt], vf[0][2 * kt + 1], vf[1][2 * kt + 1], b0, b1);
                 }
             }
@@ -240,7 +259,7 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, 2) sample_rows_tf32_kernel(con
 #pragma unroll
                 for (int nt = 0; nt < NT; ++nt) {
                     const float2 b = *(reinterpret_cast<const float2*>(T) + (kt * NT + nt) * 32 + (g & 1) * 16 + (g >> 1) * 4 + q);
-                    mma16808_tf32(acc[0][nt][0], acc[0][nt][1], acc[1][nt][0], acc[1][nt][1],
+                    mma_tf32_x<X3>(acc[0][nt][0], acc[0][nt][1], acc[1][nt][0], acc[1][nt][1],
                                   vf[0][2 * kt], vf[1][2 * kt], vf[0][2 * kt + 1], vf[1][2 * kt + 1], b.x, b.y);
                 }
             // rho_a = | t_a . R_col |

@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libtnmc.so")
 
 TNMC_OK, TNMC_EINVAL, TNMC_ENOMEM, TNMC_ECUDA, TNMC_ESTATE, TNMC_ENUMERIC = range(6)
-TNMC_F64, TNMC_F32_LOGSCALE, TNMC_F32_STORE = 0, 1, 2
+TNMC_F64, TNMC_F32_LOGSCALE, TNMC_F32_STORE, TNMC_TF32_FAST = 0, 1, 2, 3
 FLAG_NAMES = ("rho_zero", "nonfinite", "logz_nonpos", "near_threshold", "jacobi_limit", "sigma_zero",
               "reserved6", "reserved7")
 N_FLAGS = 8

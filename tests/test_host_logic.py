@@ -32,7 +32,7 @@ def test_workspace_bytes_and_argument_errors(lib):
     assert lib.tnmc_workspace_bytes(8, 1, 1, 1, 0, 0) == 0          # chi < 2
     assert lib.tnmc_workspace_bytes(8, 33, 1, 1, 0, 0) == 0         # chi > 32
     assert lib.tnmc_workspace_bytes(8, 4, 0, 1, 0, 0) == 0
-    assert lib.tnmc_workspace_bytes(8, 4, 1, 1, 3, 0) == 0          # unknown precision
+    assert lib.tnmc_workspace_bytes(8, 4, 1, 1, 4, 0) == 0          # unknown precision
     assert lib.tnmc_workspace_bytes(64, 32, 8, 8, 2, 0) == lib.tnmc_workspace_bytes(64, 32, 8, 8, 1, 0)   # both FP32 stacks
     f64, f32 = lib.tnmc_workspace_bytes(64, 32, 8, 8, 0, 0), lib.tnmc_workspace_bytes(64, 32, 8, 8, 1, 0)
     assert 0 < f32 < f64                                            # TNMC_F32_LOGSCALE halves the stack
