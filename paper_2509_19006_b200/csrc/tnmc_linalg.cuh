@@ -438,4 +438,112 @@ __device__ int jacobi_rows2(double* M, int ld, int n, double fro2, double thr2, 
     return sweep;
 }
 
+// One-sided Jacobi, third version: the same round-robin schedule as jacobi_rows2 (round R of a sweep holds the
+// pairs (R + p, R - p) mod (n-1), p = 1 .. n/2 - 1, and (n-1, R)), but the pairs are dealt to the lane groups so
+// that one row of every pair STAYS IN THE GROUP'S REGISTERS from round to round.  In the circle method a row is
+// the "plus" member of pairs p = n/2-1, ..., 1, then meets row n-1, then is the "minus" member of p = 1, ...,
+// n/2-1: a group adopts a row when it turns plus, keeps it for n/2 rounds, and writes it back after it has met
+// row n-1; only the partner row (a minus member, or row n-1) goes through shared memory each round.  That
+// halves the shared-memory traffic of a round, which is what bounds the Jacobi at chi = 32.
+// The rotation is written symmetrically (new r = cos r -+ sin r') so it does not depend on which member is held.
+// Same arguments, thresholds and return value as jacobi_rows2.
+template <int NK, int LPP>
+__device__ int jacobi_rows3(double* M, int ld, int n, double fro2, double thr2, unsigned long long* flags) {
+    const int grp = threadIdx.x / LPP, t8 = threadIdx.x % LPP;
+    const int m = n >> 1, n1 = n - 1;
+    const bool act = grp < m;
+    const unsigned gmask = ((1u << LPP) - 1u) << ((threadIdx.x & 31) & ~(LPP - 1));
+    const double rot2 = 256.0 * 4.930380657631324e-32;             // (16 eps)^2
+    const double big2 = 1e-16;                                     // (1e-8)^2
+    const double floor2 = 65536.0 * 4.930380657631324e-32 * fro2;  // (256 eps |M|_F)^2
+    const int c0 = 2 * t8;
+    int sweep = 0;
+    for (; sweep < 60; ++sweep) {
+        int big = 0;
+        // state of this group at round 0: age = rounds since it adopted its row, delta = m - 1 - age = the p of
+        // its pair (0: the row meets row n-1); own = delta, pm = (round - delta) mod (n-1) = the minus member
+        int age = grp == 0 ? 0 : m - grp;
+        int own = m - 1 - age;
+        int pm = own == 0 ? 0 : n1 - own;
+        double2 ov[NK];
+        if (act) {
+#pragma unroll
+            for (int k = 0; k < NK; ++k) ov[k] = *reinterpret_cast<const double2*>(M + (size_t)own * ld + c0 + 2 * LPP * k);
+        }
+        for (int round = 0; round < n1; ++round) {
+            if (act) {
+                const bool last = age == m - 1;                    // delta == 0: partner is row n-1
+                const int prt = last ? n1 : pm;
+                double* y = M + (size_t)prt * ld;
+                double2 pv[NK];
+#pragma unroll
+                for (int k = 0; k < NK; ++k) pv[k] = *reinterpret_cast<const double2*>(y + c0 + 2 * LPP * k);
+                double ao = 0.0, ap = 0.0, g = 0.0, ao1 = 0.0, ap1 = 0.0, g1 = 0.0;
+#pragma unroll
+                for (int k = 0; k < NK; ++k) {
+                    ao = fma(ov[k].x, ov[k].x, ao);  ao1 = fma(ov[k].y, ov[k].y, ao1);
+                    ap = fma(pv[k].x, pv[k].x, ap);  ap1 = fma(pv[k].y, pv[k].y, ap1);
+                    g = fma(ov[k].x, pv[k].x, g);    g1 = fma(ov[k].y, pv[k].y, g1);
+                }
+                ao += ao1; ap += ap1; g += g1;
+#pragma unroll
+                for (int o = LPP / 2; o > 0; o >>= 1) {
+                    ao += __shfl_xor_sync(gmask, ao, o);
+                    ap += __shfl_xor_sync(gmask, ap, o);
+                    g += __shfl_xor_sync(gmask, g, o);
+                }
+                const double g2 = g * g, ab = ao * ap;
+                if (ao > thr2 && ap > thr2 && g2 > rot2 * ab) {
+                    const double mx = ao > ap ? ao : ap;
+                    big |= (g2 > big2 * ab) && (g2 > floor2 * mx);
+                    // x = the row of smaller index, y = the other: d = |y|^2 - |x|^2, x' = cos x - sin y, y' = cos y + sin x
+                    const bool own_is_x = own < prt;
+                    const double dd = own_is_x ? ap - ao : ao - ap;
+                    const double g24 = 4.0 * g2;
+                    const double h2 = fma(dd, dd, g24);
+                    const double u = fabs(dd) + h2 * fast_rsqrt(h2);
+                    const double w = fast_rsqrt(fma(u, u, g24));
+                    const double cs = u * w;
+                    double sn = 2.0 * g * w;
+                    if (dd < 0.0) sn = -sn;
+                    const double so = own_is_x ? -sn : sn;         // own' = cos own + so prt,  prt' = cos prt - so own
+#pragma unroll
+                    for (int k = 0; k < NK; ++k) {
+                        double2 on, pn;
+                        on.x = fma(cs, ov[k].x, so * pv[k].x);  pn.x = fma(cs, pv[k].x, -so * ov[k].x);
+                        on.y = fma(cs, ov[k].y, so * pv[k].y);  pn.y = fma(cs, pv[k].y, -so * ov[k].y);
+                        ov[k] = on;
+                        *reinterpret_cast<double2*>(y + c0 + 2 * LPP * k) = pn;
+                    }
+                }
+                if (last) {     // the held row has met every other row: back to shared memory, adopt the next one
+                    double* x = M + (size_t)own * ld;
+#pragma unroll
+                    for (int k = 0; k < NK; ++k) *reinterpret_cast<double2*>(x + c0 + 2 * LPP * k) = ov[k];
+                    age = 0;
+                    own += m;      if (own >= n1) own -= n1;
+                    pm += m + 1;   if (pm >= n1) pm -= n1;
+                } else {
+                    ++age;
+                    pm += 2;       if (pm >= n1) pm -= n1;
+                }
+            }
+            __syncthreads();
+            if (act && age == 0 && round + 1 < n1) {   // adopt: the row that was the minus member of pair n/2-1
+#pragma unroll
+                for (int k = 0; k < NK; ++k) ov[k] = *reinterpret_cast<const double2*>(M + (size_t)own * ld + c0 + 2 * LPP * k);
+            }
+        }
+        // end of sweep: every held row goes back (a group that has just released its row holds nothing new yet)
+        if (act && age != 0) {
+            double* x = M + (size_t)own * ld;
+#pragma unroll
+            for (int k = 0; k < NK; ++k) *reinterpret_cast<double2*>(x + c0 + 2 * LPP * k) = ov[k];
+        }
+        if (!__syncthreads_or(big)) { ++sweep; break; }
+    }
+    if (sweep >= 60 && threadIdx.x == 0) raise_flag(flags, FLAG_JACOBI_LIMIT);
+    return sweep;
+}
+
 }  // namespace tnmc
