@@ -67,7 +67,7 @@ struct BuildCfg {
     // L2-resident global scratch for P = 32, which brings the CTA to 88 KB: two CTAs per SM.
     static constexpr bool M0_GLOBAL = P >= 32;
     static constexpr int CTAS_PER_SM = P >= 32 ? 2 : 3;
-    static constexpr bool JACOBI_HELD_ROW = P >= 32;     // jacobi_rows3 (measured faster at chi = 32, slower at chi = 16)
+    static constexpr bool JACOBI_HELD_ROW = P >= 32;     // jacobi_rows4 (measured faster at chi = 32, slower at chi = 16)
     static constexpr int Z_OFF = Y_OFF + Y_SZ;            // D*D   : M before rotation (SVD sweep), P <= 16 only
     static constexpr int U_OFF = Z_OFF + (M0_GLOBAL ? 0 : D * D);   // D*LDU : C_a (QR sweep); carried Pc / M V_k (SVD sweep)
     static constexpr int S_OFF = U_OFF + D * LDU;         // D + 24 + D + 40 : tau / QRCP scratch / sigma / reduction scratch
@@ -270,13 +270,14 @@ __global__ void __launch_bounds__(BuildCfg<P>::NT, BuildCfg<P>::CTAS_PER_SM) bui
             __syncthreads();
             const double thr2 = fro2 * 1e-30;      // sigma <= 1e-15 |M|_F: below the numerical rank
             PROF(4);
-            // chi = 32: a round is bound by shared-memory traffic and FP64 issue -> one row of each pair held in registers
-            // (jacobi_rows3: C3 build 6.48 -> 6.06 s); chi <= 16: one warp per scheduler, bound by the latency of the
-            // dependent chain, where the extra bookkeeping costs more than the saved loads (C2 build 93 -> 100 ms): jacobi_rows2
+            // chi = 32: one row of each pair held in registers, norms carried (jacobi_rows4: C3 build 6.48 -> 5.97 s);
+            // chi <= 16: one warp per scheduler, bound by the latency of the dependent chain, where the bookkeeping of
+            // the held row costs more than the loads it saves (C2 build 93 -> 100 ms): jacobi_rows2
             constexpr int JNK = (D + 2 * Cfg::LPP - 1) / (2 * Cfg::LPP);
             int nsw = 0;
             if (nrow >= 2) {
-                if constexpr (Cfg::JACOBI_HELD_ROW) nsw = jacobi_rows3<JNK, Cfg::LPP>(sMj, LDM, nrow, fro2, thr2, args.flags);
+                static_assert(JNK * 2 * Cfg::LPP < LDM, "the carried norm of a row lives in the spare column after its padded width");
+                if constexpr (Cfg::JACOBI_HELD_ROW) nsw = jacobi_rows4<JNK, Cfg::LPP>(sMj, LDM, JNK * 2 * Cfg::LPP, nrow, fro2, thr2, args.flags);
                 else nsw = jacobi_rows2<JNK, Cfg::LPP>(sMj, LDM, nrow, fro2, thr2, args.flags);
             }
             PROF(5);

@@ -41,6 +41,15 @@ __device__ __forceinline__ double fast_rsqrt(double x) {
     r = r * fma(-hx * r, r, 1.5);
     return r;
 }
+// one Newton step: relative error ~ 1e-13.  Enough for the Jacobi rotation: an error in w scales both rows of the
+// pair alike (directions unchanged), an error in h tilts the angle by 1e-13 of itself (left to the next sweep).
+__device__ __forceinline__ double fast_rsqrt1(double x) {
+    double r;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    const double hx = 0.5 * x;
+    r = r * fma(-hx * r, r, 1.5);
+    return r;
+}
 __device__ __forceinline__ double fast_rcp(double x) {
     double r;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
@@ -414,8 +423,8 @@ __device__ int jacobi_rows2(double* M, int ld, int n, double fro2, double thr2, 
                     const double dd = b - a;
                     const double g24 = 4.0 * g2;
                     const double h2 = fma(dd, dd, g24);
-                    const double u = fabs(dd) + h2 * fast_rsqrt(h2);
-                    const double w = fast_rsqrt(fma(u, u, g24));
+                    const double u = fabs(dd) + h2 * fast_rsqrt1(h2);
+                    const double w = fast_rsqrt1(fma(u, u, g24));
                     const double cs = u * w;
                     double sn = 2.0 * g * w;
                     if (dd < 0.0) sn = -sn;
@@ -438,17 +447,23 @@ __device__ int jacobi_rows2(double* M, int ld, int n, double fro2, double thr2, 
     return sweep;
 }
 
-// One-sided Jacobi, third version: the same round-robin schedule as jacobi_rows2 (round R of a sweep holds the
-// pairs (R + p, R - p) mod (n-1), p = 1 .. n/2 - 1, and (n-1, R)), but the pairs are dealt to the lane groups so
-// that one row of every pair STAYS IN THE GROUP'S REGISTERS from round to round.  In the circle method a row is
-// the "plus" member of pairs p = n/2-1, ..., 1, then meets row n-1, then is the "minus" member of p = 1, ...,
-// n/2-1: a group adopts a row when it turns plus, keeps it for n/2 rounds, and writes it back after it has met
-// row n-1; only the partner row (a minus member, or row n-1) goes through shared memory each round.  That
-// halves the shared-memory traffic of a round, which is what bounds the Jacobi at chi = 32.
-// The rotation is written symmetrically (new r = cos r -+ sin r') so it does not depend on which member is held.
-// Same arguments, thresholds and return value as jacobi_rows2.
+// One-sided Jacobi with a HELD ROW (used at chi = 32).  The same round-robin schedule as jacobi_rows2 (round R of a
+// sweep holds the pairs (R + p, R - p) mod (n-1), p = 1 .. n/2 - 1, and (n-1, R)), but the pairs are dealt to the
+// lane groups so that one row of every pair STAYS IN THE GROUP'S REGISTERS from round to round.  In the circle
+// method a row is the "plus" member of pairs p = n/2-1, ..., 1, then meets row n-1, then is the "minus" member of
+// p = 1, ..., n/2-1: a group adopts a row when it turns plus, keeps it for n/2 rounds, and writes it back after it
+// has met row n-1; only the partner row (a minus member, or row n-1) goes through shared memory each round: half
+// the shared-memory traffic of a round.  The rotation is written symmetrically (new r = cos r -+ sin r') so it does
+// not depend on which member is held.
+// The squared row norms are CARRIED instead of re-summed every round: a rotation by the Jacobi angle changes them
+// by exactly -+ t g (t = tan, g = the pair's dot product; the larger grows, the smaller shrinks, by 2 g^2 / u), so
+// a round sums one dot product instead of three.  The held row's norm travels in a register, a moving row's norm in
+// the spare column `nslot` of its shared-memory row (nslot >= the padded width, < ld); all norms are summed afresh
+// at the start of every sweep, so the carried values are at most n-1 updates (a few 1e-15 relative) old -- they
+// only steer the rotation angle and the thresholds; the singular values are summed from the rows afterwards.
+// Otherwise the same arguments, thresholds and return value as jacobi_rows2.
 template <int NK, int LPP>
-__device__ int jacobi_rows3(double* M, int ld, int n, double fro2, double thr2, unsigned long long* flags) {
+__device__ int jacobi_rows4(double* M, int ld, int nslot, int n, double fro2, double thr2, unsigned long long* flags) {
     const int grp = threadIdx.x / LPP, t8 = threadIdx.x % LPP;
     const int m = n >> 1, n1 = n - 1;
     const bool act = grp < m;
@@ -466,9 +481,28 @@ __device__ int jacobi_rows3(double* M, int ld, int n, double fro2, double thr2, 
         int own = m - 1 - age;
         int pm = own == 0 ? 0 : n1 - own;
         double2 ov[NK];
+        double ao = 0.0;     // carried squared norm of the held row
+        if (act) {           // fresh norms of rows 2 grp, 2 grp + 1 into their slots
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const double* x = M + (size_t)(2 * grp + h) * ld;
+                double s0 = 0.0, s1 = 0.0;
+#pragma unroll
+                for (int k = 0; k < NK; ++k) {
+                    const double2 v = *reinterpret_cast<const double2*>(x + c0 + 2 * LPP * k);
+                    s0 = fma(v.x, v.x, s0);  s1 = fma(v.y, v.y, s1);
+                }
+                s0 += s1;
+#pragma unroll
+                for (int o = LPP / 2; o > 0; o >>= 1) s0 += __shfl_xor_sync(gmask, s0, o);
+                if (t8 == 0) M[(size_t)(2 * grp + h) * ld + nslot] = s0;
+            }
+        }
+        __syncthreads();
         if (act) {
 #pragma unroll
             for (int k = 0; k < NK; ++k) ov[k] = *reinterpret_cast<const double2*>(M + (size_t)own * ld + c0 + 2 * LPP * k);
+            ao = M[(size_t)own * ld + nslot];
         }
         for (int round = 0; round < n1; ++round) {
             if (act) {
@@ -478,20 +512,13 @@ __device__ int jacobi_rows3(double* M, int ld, int n, double fro2, double thr2, 
                 double2 pv[NK];
 #pragma unroll
                 for (int k = 0; k < NK; ++k) pv[k] = *reinterpret_cast<const double2*>(y + c0 + 2 * LPP * k);
-                double ao = 0.0, ap = 0.0, g = 0.0, ao1 = 0.0, ap1 = 0.0, g1 = 0.0;
+                const double ap = y[nslot];
+                double g = 0.0, g1 = 0.0;
 #pragma unroll
-                for (int k = 0; k < NK; ++k) {
-                    ao = fma(ov[k].x, ov[k].x, ao);  ao1 = fma(ov[k].y, ov[k].y, ao1);
-                    ap = fma(pv[k].x, pv[k].x, ap);  ap1 = fma(pv[k].y, pv[k].y, ap1);
-                    g = fma(ov[k].x, pv[k].x, g);    g1 = fma(ov[k].y, pv[k].y, g1);
-                }
-                ao += ao1; ap += ap1; g += g1;
+                for (int k = 0; k < NK; ++k) { g = fma(ov[k].x, pv[k].x, g);  g1 = fma(ov[k].y, pv[k].y, g1); }
+                g += g1;
 #pragma unroll
-                for (int o = LPP / 2; o > 0; o >>= 1) {
-                    ao += __shfl_xor_sync(gmask, ao, o);
-                    ap += __shfl_xor_sync(gmask, ap, o);
-                    g += __shfl_xor_sync(gmask, g, o);
-                }
+                for (int o = LPP / 2; o > 0; o >>= 1) g += __shfl_xor_sync(gmask, g, o);
                 const double g2 = g * g, ab = ao * ap;
                 if (ao > thr2 && ap > thr2 && g2 > rot2 * ab) {
                     const double mx = ao > ap ? ao : ap;
@@ -501,12 +528,18 @@ __device__ int jacobi_rows3(double* M, int ld, int n, double fro2, double thr2, 
                     const double dd = own_is_x ? ap - ao : ao - ap;
                     const double g24 = 4.0 * g2;
                     const double h2 = fma(dd, dd, g24);
-                    const double u = fabs(dd) + h2 * fast_rsqrt(h2);
-                    const double w = fast_rsqrt(fma(u, u, g24));
+                    const double u = fabs(dd) + h2 * fast_rsqrt1(h2);
+                    const double w = fast_rsqrt1(fma(u, u, g24));
                     const double cs = u * w;
                     double sn = 2.0 * g * w;
                     if (dd < 0.0) sn = -sn;
                     const double so = own_is_x ? -sn : sn;         // own' = cos own + so prt,  prt' = cos prt - so own
+                    // norms: |x'|^2 = |x|^2 - t g, |y'|^2 = |y|^2 + t g with t g = sign(d) 2 g^2 / u
+                    const double qn = 0.5 * g24 * fast_rcp(u);
+                    const bool own_grows = own_is_x == (dd < 0.0);
+                    const double apn = own_grows ? ap - qn : ap + qn;
+                    ao = own_grows ? ao + qn : ao - qn;
+                    if (t8 == 0) y[nslot] = apn;
 #pragma unroll
                     for (int k = 0; k < NK; ++k) {
                         double2 on, pn;
@@ -520,6 +553,7 @@ __device__ int jacobi_rows3(double* M, int ld, int n, double fro2, double thr2, 
                     double* x = M + (size_t)own * ld;
 #pragma unroll
                     for (int k = 0; k < NK; ++k) *reinterpret_cast<double2*>(x + c0 + 2 * LPP * k) = ov[k];
+                    if (t8 == 0) x[nslot] = ao;
                     age = 0;
                     own += m;      if (own >= n1) own -= n1;
                     pm += m + 1;   if (pm >= n1) pm -= n1;
@@ -532,6 +566,7 @@ __device__ int jacobi_rows3(double* M, int ld, int n, double fro2, double thr2, 
             if (act && age == 0 && round + 1 < n1) {   // adopt: the row that was the minus member of pair n/2-1
 #pragma unroll
                 for (int k = 0; k < NK; ++k) ov[k] = *reinterpret_cast<const double2*>(M + (size_t)own * ld + c0 + 2 * LPP * k);
+                ao = M[(size_t)own * ld + nslot];
             }
         }
         // end of sweep: every held row goes back (a group that has just released its row holds nothing new yet)
