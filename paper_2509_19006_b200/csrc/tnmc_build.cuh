@@ -214,9 +214,23 @@ __global__ void __launch_bounds__(BuildCfg<P>::NT, BuildCfg<P>::CTAS_PER_SM) bui
             } else {
                 // M = [Q_0 Pc_0 | Q_1 Pc_1]: reflectors of block a applied to [Pc_a; 0]
                 const int p = sq[c + 1] >> 1;
-                for (int t = tid; t < 2 * q * p; t += NT) {
-                    const int x = t % q, z = (t / q) % p, a = t / (q * p);
-                    sY[(size_t)(a * P + z) * LDX + x] = Qin[(size_t)(a * P + z) * LDX + x];
+                // the p reflector columns of a block are contiguous in the scratch image of X: flat copy, four loads in
+                // flight per thread (rows >= q of a column were never written and are never read)
+                for (int a = 0; a < 2; ++a) {
+                    const double* src = Qin + (size_t)a * P * LDX;
+                    double* dst = sY + (size_t)a * P * LDX;
+                    const int nflat = p * LDX;
+                    for (int t = tid; t < nflat; t += 4 * NT) {
+                        const int t1 = t + NT, t2 = t + 2 * NT, t3 = t + 3 * NT;
+                        const double v0 = src[t];
+                        const double v1 = t1 < nflat ? src[t1] : 0.0;
+                        const double v2 = t2 < nflat ? src[t2] : 0.0;
+                        const double v3 = t3 < nflat ? src[t3] : 0.0;
+                        dst[t] = v0;
+                        if (t1 < nflat) dst[t1] = v1;
+                        if (t2 < nflat) dst[t2] = v2;
+                        if (t3 < nflat) dst[t3] = v3;
+                    }
                 }
                 for (int t = tid; t < 2 * p; t += NT) {
                     const int z = t % p, a = t / p;
