@@ -231,7 +231,14 @@ __device__ void householder_qr_g(double* X, int ld, int m, int n, double* tau, i
                 double bet, t1, scale;
                 reflector_from_norm(col[j + 1], below2, bet, t1, scale);
                 __syncwarp(qmask);
-                for (int i = j + 2 + rg; i < m; i += 4) col[i] *= scale;
+                {   // scale the new reflector: this quad alone is between the others and the step's barrier, so the
+                    // loads go out together (elementwise, bit-identical to the plain loop)
+                    double tmp[MAXK];
+#pragma unroll
+                    for (int k = 0; k < MAXK; ++k) { const int i = j + 2 + rg + 4 * k; tmp[k] = i < m ? col[i] : 0.0; }
+#pragma unroll
+                    for (int k = 0; k < MAXK; ++k) { const int i = j + 2 + rg + 4 * k; if (i < m) col[i] = tmp[k] * scale; }
+                }
                 if (rg == 0) { col[j + 1] = bet; tau[j + 1] = t1; }
             }
         }
