@@ -1,0 +1,131 @@
+"""GPU parity at the BASELINE.json configs' OWN sizes: the CUDA path (through the C ABI binding) against the
+oracle's stored outputs tests/golden/config_<C2..C5>.npz (written by tests/golden/make_config_golden.py from
+oracle/ only).  Compared element by element per (beta, disorder): log Z, the sampled spins (bit-exact off the chains
+that came within `tol` of a threshold), log q, energies (bit-exact), the stored conditionals; the tolerance policy and
+the record of the achieved deviations are tests/parity_report.py's.  C4/C5 run with row checkpoints + segment
+recomputation (a-6), as bench.py runs them."""
+import os
+
+import numpy as np
+import pytest
+
+from tnmc_workloads import make_couplings
+
+from bitpack import unpack
+import parity_report as pr
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+GOLD = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+@pytest.fixture(scope="module")
+def tn():
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    from paper_2509_19006_b200 import tnmc
+    return tnmc
+
+
+def _groups(ds):
+    """runs of consecutive disorder indices -> one GPU context each"""
+    out, run = [], [0]
+    for i in range(1, len(ds)):
+        if ds[i] == ds[i - 1] + 1:
+            run.append(i)
+        else:
+            out.append(run)
+            run = [i]
+    out.append(run)
+    return out
+
+
+def _run_case(tn, g, name, bi, ckpt, prec=None, lz_only=False, only=None):
+    """one beta of a golden file: GPU contexts over exactly the stored disorders, compared with the file"""
+    dev = torch.device("cuda:0")
+    L, chi, beta = int(g["L"]), int(g["chi"]), float(g["betas"][bi])
+    inst_seed, seed = int(g["inst_seed"]), int(g["seed"])
+    n_s = g["logq"].shape[2]
+    prob_rows = g["prob_rows"]
+    n_p = g["probs"].shape[2]
+    ds = [int(x) for x in g["disorders"]]
+    bad = []
+    for grp in _groups(ds):
+        if only is not None:
+            grp = [i for i in grp if i in only]
+            if not grp:
+                continue
+        d0, nd = ds[grp[0]], len(grp)
+        Jr, Jd = make_couplings(L, nd, inst_seed, first_disorder=d0)
+        kw = {} if prec is None else {"prec": prec}
+        ctx = tn.Context(L, chi, beta, torch.from_numpy(Jr).to(dev), torch.from_numpy(Jd).to(dev), n_s,
+                         first_disorder=d0, ckpt_stride=ckpt, **kw)
+        logZ = ctx.tnmc_build_envs().cpu().numpy()
+        if not lz_only:
+            probs = torch.zeros((nd, n_p, L, L), dtype=torch.float64, device=dev)
+            bits_p, logq_p = ctx.tnmc_sample(n_p, seed, probs=probs)
+            bits, logq = ctx.tnmc_sample(n_s, seed)
+            assert torch.equal(bits[:, :n_p], bits_p) and torch.equal(logq[:, :n_p], logq_p)
+            E = ctx.tnmc_energy(bits).cpu().numpy()
+            flags = ctx.tnmc_get_flags()
+            assert flags["nonfinite"] == 0 and flags["jacobi_limit"] == 0 and flags["rho_zero"] == 0 and flags["logz_nonpos"] == 0
+            bits = bits.cpu().numpy().view(np.uint32)
+            logq = logq.cpu().numpy()
+            probs = probs.cpu().numpy()[:, :, prob_rows, :]
+        ctx.close()
+        for j, di in enumerate(grp):
+            case = f"{name} beta={beta} d={ds[di]}" + (f" prec={prec}" if prec is not None else "")
+            lz = float(g["logZ"][bi, di])
+            if lz_only:     # reduced-precision modes: north_star's 1e-4 on log Z
+                if not pr.check(case, "logZ_rel", abs(logZ[j] - lz) / abs(lz), 1e-4, do_assert=False):
+                    bad.append(case)
+                continue
+            ok = pr.check(case, "logZ_rel", abs(logZ[j] - lz) / abs(lz), 1e-10, float(g["floor_logZ"][bi, di]) / abs(lz), do_assert=False)
+            fl_p, fl_q = float(g["floor_p"][bi, di]), float(g["floor_logq"][bi, di])
+            tol_p, _ = pr.tolerance(1e-9, fl_p)
+            same = (bits[j] == g["cfg_bits"][bi, di]).all(axis=(1, 2))
+            near = g["min_margin"][bi, di] < tol_p             # a draw too close to its threshold to call
+            pr.record(case=case, quantity="chains", n=int(n_s), identical=int(same.sum()), near_threshold=int(near.sum()),
+                      ok=bool((same | near).all()))
+            ok &= bool((same | near).all())
+            good = same & ~near
+            if good.any():
+                o_logq = g["logq"][bi, di]
+                scale = max(1.0, float(np.abs(o_logq).max()))
+                ok &= pr.check(case, "logq_rel", np.abs(logq[j][good] - o_logq[good]).max() / scale, 1e-9, fl_q / scale, do_assert=False)
+                ok &= bool((E[j][good] == g["E"][bi, di][good]).all())
+                gp = good[:n_p]
+                if gp.any():
+                    ok &= pr.check(case, "p_abs", np.abs(probs[j][gp] - g["probs"][bi, di][gp]).max(), 1e-9, fl_p, do_assert=False)
+            if not ok:
+                bad.append(case)
+    return bad
+
+
+def test_config_c2_all_disorders(tn):
+    """C2 in full: every one of the 100 disorders at the three betas, 32 samples each, against the stored oracle."""
+    g = np.load(os.path.join(GOLD, "config_C2.npz"))
+    bad = []
+    for bi in range(len(g["betas"])):
+        bad += _run_case(tn, g, "C2", bi, 0)
+    assert not bad, bad
+
+
+def test_config_c3_golden(tn):
+    g = np.load(os.path.join(GOLD, "config_C3.npz"))
+    bad = _run_case(tn, g, "C3", 0, 0)
+    bad += _run_case(tn, g, "C3", 0, 0, prec=tn.TNMC_F32_LOGSCALE, lz_only=True, only=[0])
+    bad += _run_case(tn, g, "C3", 0, 0, prec=tn.TNMC_F32_STORE, lz_only=True, only=[0])
+    assert not bad, bad
+
+
+def test_config_c4_golden(tn):
+    g = np.load(os.path.join(GOLD, "config_C4.npz"))
+    bad = _run_case(tn, g, "C4", 0, 23)
+    assert not bad, bad
+
+
+def test_config_c5_golden(tn):
+    g = np.load(os.path.join(GOLD, "config_C5.npz"))
+    bad = _run_case(tn, g, "C5", 0, 32)
+    assert not bad, bad
