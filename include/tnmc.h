@@ -217,6 +217,20 @@ tnmc_status tnmc_observables_real(tnmc_ctx* ctx, int dis_begin, int dis_count, i
                                   const uint32_t* cfg_bits, const double* E, const uint8_t* accepted,
                                   int32_t* M, double* cur_E, int32_t* cur_M, double* sums);
 
+/* tnmc_observables for callers that cannot allocate device memory (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): the same two kernels, with the per-proposal magnetisations M -- the
+ * scratch between them -- held in a file-scope device array of the library instead of a caller buffer.  The call
+ * makes no cudaMalloc / cudaFree / allocating library call.  +-J contexts only.
+ *   limit: dis_count * n_samples <= tnmc_observables_static_max() (2^20 proposals; the array is 4 MiB of device
+ *   memory on every GPU that loads the library, held until exit).  Larger calls return TNMC_EINVAL.
+ *   cfg_bits, E, accepted, cur_E, cur_M, sums: as tnmc_observables (no M output).
+ * All calls on one device share the array: calls that may overlap on the GPU (different streams, no ordering) race.
+ * Nothing in it has to start at zero -- each call overwrites the entries it reads. */
+size_t tnmc_observables_static_max(void);
+tnmc_status tnmc_observables_static(tnmc_ctx* ctx, int dis_begin, int dis_count, int n_samples,
+                                    const uint32_t* cfg_bits, const int32_t* E, const uint8_t* accepted,
+                                    int32_t* cur_E, int32_t* cur_M, double* sums);
+
 /* One whole pass for host callers: copies Jr/Jd (host, int8 (n_dis,L,L)) to the device, builds
  * the environments, samples, computes energies, runs the Metropolis scan on fresh chains and
  * copies the results back.  All device memory comes from `workspace`

@@ -2,6 +2,7 @@
 // Every step of the hot path runs in the kernels of tnmc_build.cuh / tnmc_sample.cuh /
 // tnmc_energy.cuh; nothing here computes on the host and there is no CPU fallback.
 #include <cmath>
+#include <mutex>
 
 #include "tnmc_ctx.cuh"
 
@@ -364,6 +365,58 @@ extern "C" tnmc_status tnmc_observables_real(tnmc_ctx* ctx, int dis_begin, int d
                                              const uint32_t* cfg_bits, const double* E, const uint8_t* accepted,
                                              int32_t* M, double* cur_E, int32_t* cur_M, double* sums) {
     return observables_impl<double>(ctx, "tnmc_observables_real", dis_begin, dis_count, n_samples, cfg_bits, E, accepted, M, cur_E, cur_M, sums);
+}
+
+// ---------------------------------------------------------------------------------------------
+// tnmc_observables_static: tnmc_observables with the per-proposal magnetisations -- the scratch that
+// magnetisation_kernel writes and observables_kernel reads -- in a file-scope device array instead of
+// a caller buffer.  For callers that cannot allocate (CUDA graph capture, serving loops): the call
+// allocates nothing on host-visible CUDA APIs (no cudaMalloc / cudaFree / allocating library routine).
+// ---------------------------------------------------------------------------------------------
+#define TNMC_STATIC_M_MAX (1 << 20)                       /* int32 entries: 4 MiB per device that loads the library */
+static __device__ __align__(256) int32_t g_static_M[TNMC_STATIC_M_MAX];
+
+namespace {
+constexpr int STATIC_MAX_DEVICES = 64;
+int32_t* g_static_M_ptr[STATIC_MAX_DEVICES] = {nullptr};   // device address of g_static_M, per device
+std::mutex g_static_mu;
+}  // namespace
+
+// Device address of g_static_M on the CURRENT device (in host code the symbol itself is only a stand-in):
+// resolved once per device with that device current.
+static cudaError_t static_M_address(int32_t** out) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_M_ptr[dev]) {
+        void* p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_static_M);
+        if (e != cudaSuccess) return e;
+        g_static_M_ptr[dev] = reinterpret_cast<int32_t*>(p);
+    }
+    *out = g_static_M_ptr[dev];
+    return cudaSuccess;
+}
+
+extern "C" size_t tnmc_observables_static_max(void) { return (size_t)TNMC_STATIC_M_MAX; }
+
+extern "C" tnmc_status tnmc_observables_static(tnmc_ctx* ctx, int dis_begin, int dis_count, int n_samples,
+                                               const uint32_t* cfg_bits, const int32_t* E, const uint8_t* accepted,
+                                               int32_t* cur_E, int32_t* cur_M, double* sums) {
+    tnmc_status st = check_range(ctx, "tnmc_observables_static", dis_begin, dis_count, n_samples);
+    if (st != TNMC_OK) return st;
+    if (ctx->plan.real_j) return fail(ctx, TNMC_ESTATE, "tnmc_observables_static: +-J contexts only");
+    if ((long long)dis_count * n_samples > (long long)TNMC_STATIC_M_MAX)
+        return fail(ctx, TNMC_EINVAL, "tnmc_observables_static: dis_count * n_samples exceeds the static scratch ("
+                                      + std::to_string(TNMC_STATIC_M_MAX) + " proposals); use tnmc_observables");
+    int32_t* M = nullptr;
+    cudaError_t e = static_M_address(&M);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "tnmc_observables_static: cudaGetSymbolAddress");
+    // every entry the scan reads is overwritten by magnetisation_kernel first: nothing has to start at zero
+    return observables_impl<int32_t>(ctx, "tnmc_observables_static", dis_begin, dis_count, n_samples, cfg_bits, E, accepted,
+                                     M, cur_E, cur_M, sums);
 }
 
 // ---------------------------------------------------------------------------------------------

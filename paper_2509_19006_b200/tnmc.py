@@ -52,6 +52,10 @@ def _load():
     lib.tnmc_observables.argtypes = [vp, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp]
     lib.tnmc_observables_real.restype = i32
     lib.tnmc_observables_real.argtypes = [vp, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp]
+    lib.tnmc_observables_static_max.restype = sz
+    lib.tnmc_observables_static_max.argtypes = []
+    lib.tnmc_observables_static.restype = i32
+    lib.tnmc_observables_static.argtypes = [vp, i32, i32, i32, vp, vp, vp, vp, vp, vp]
     lib.tnmc_run_host_workspace_bytes.restype = sz
     lib.tnmc_run_host_workspace_bytes.argtypes = [i32, i32, i32, i32, i32, i32]
     lib.tnmc_run_host.restype = i32
@@ -212,6 +216,15 @@ class Context:
                                     _ptr(accepted, torch.uint8), _ptr(M, torch.int32), _ptr(state[0], et),
                                     _ptr(state[1], torch.int32), _ptr(sums, torch.float64)), self.h)
         return M, state, sums
+
+    def tnmc_observables_static(self, cfg_bits, E, accepted, state, sums, dis_begin=0):
+        """tnmc_observables without any allocation: `state` = (cur_E, cur_M) and `sums` are caller tensors, the
+        magnetisation scratch is the library's static device array (limit tnmc_observables_static_max proposals)."""
+        dis_count, n_samples = E.shape
+        _check(lib.tnmc_observables_static(self.h, dis_begin, dis_count, n_samples, _ptr(cfg_bits, torch.int32),
+                                           _ptr(E, torch.int32), _ptr(accepted, torch.uint8), _ptr(state[0], torch.int32),
+                                           _ptr(state[1], torch.int32), _ptr(sums, torch.float64)), self.h)
+        return state, sums
 
     # -- inspection -----------------------------------------------------------------------------
     def tnmc_get_flags(self):
