@@ -8,6 +8,13 @@ rejected steps re-counting the state they stayed on.  Observables per configurat
   E   Eq. 1, integer
   M   = sum_i s_i (magnetisation, integer in [-N, N])
 accumulated as the five sums  sum E, sum E^2, sum M, sum |M|, sum M^2  over the steps of a chunk.
+
+Replica overlap (the spin-glass order parameter; the +-J Edwards-Anderson model of PAPER.md:282-286 has
+<M> = 0 by symmetry, so the overlap between two independent replicas of the SAME disorder is the observable
+that carries the physics):  q = sum_i s_i^a s_i^b  (integer in [-N, N]; q/N is the usual normalisation).
+Two independent Metropolis chains a, b (different Philox sample ranges or seeds) are walked step by step;
+at step n each sits on its last accepted proposal, q_n is the overlap of the two current states, and the
+sums  sum q, sum |q|, sum q^2  are accumulated like the five above (same reading G19).
 """
 import numpy as np
 
@@ -46,3 +53,30 @@ def chain_sums_real(E, M, accepted, cur_E=0.0, cur_M=0):
         s[3] += abs(cur_M)
         s[4] += cur_M * cur_M
     return s, cur_E, cur_M
+
+
+def overlap(cfg_a, cfg_b):
+    """q = sum_i s_i^a s_i^b for cfg (..., L, L) in {0,1}: N - 2 * (number of sites where the two differ)."""
+    a = 2 * np.asarray(cfg_a, dtype=np.int64) - 1
+    b = 2 * np.asarray(cfg_b, dtype=np.int64) - 1
+    return (a * b).sum(axis=(-1, -2))
+
+
+def replica_overlap(cfg_a, acc_a, cfg_b, acc_b, cur_a=None, cur_b=None):
+    """cfg_x: (n, L, L) proposals of chain x, acc_x: (n,) Metropolis flags of chain x (flag 1 on the proposal that
+    initialises an empty chain); cur_x: (L, L) state of chain x entering the chunk (used until its first flag 1).
+    Returns (q_steps (n,) int64, sums [sum q, sum |q|, sum q^2] as Python ints, cur_a, cur_b)."""
+    n = len(acc_a)
+    q = np.zeros(n, dtype=np.int64)
+    s = [0, 0, 0]
+    for i in range(n):
+        if acc_a[i]:
+            cur_a = np.asarray(cfg_a[i])
+        if acc_b[i]:
+            cur_b = np.asarray(cfg_b[i])
+        qi = int(overlap(cur_a, cur_b))
+        q[i] = qi
+        s[0] += qi
+        s[1] += abs(qi)
+        s[2] += qi * qi
+    return q, s, cur_a, cur_b

@@ -67,3 +67,66 @@ def test_exact_chi_chain_reproduces_boltzmann_averages():
                                      (s[4] / n_s, (Pb * M_all ** 2).sum(), (Pb * M_all.astype(float) ** 4).sum())):
         sigma = np.sqrt(max(exact_sq - exact_val ** 2, 1e-12) / n_s)
         assert abs(est - exact_val) < 4.5 * sigma
+
+
+def test_overlap_definition_and_hand_worked_chain():
+    L = 3
+    up = np.ones((L, L), dtype=np.int8)
+    assert observables.overlap(up, up) == 9 and observables.overlap(up, 1 - up) == -9
+    c = up.copy(); c[0, 1] = 0; c[2, 2] = 0                      # differs from `up` on two sites
+    assert observables.overlap(up, c) == 9 - 4 and observables.overlap(c, up) == 5
+    assert observables.overlap(c, c) == 9
+    d = up.copy(); d[0, 1] = 0; d[1, 1] = 0                      # c and d differ on (2,2) and (1,1)
+    assert observables.overlap(c, d) == 9 - 4
+    # two chains, worked by hand: chain a proposals (up, c, d), flags 1 0 1 -> states up, up, d
+    #                             chain b proposals (c, c, up), flags 1 1 0 -> states c, c, c
+    q, s, ca, cb = observables.replica_overlap([up, c, d], [1, 0, 1], [c, c, up], [1, 1, 0])
+    assert list(q) == [5, 5, 5] and s == [15, 15, 75]            # up.c = 5, up.c = 5, d.c = 5
+    assert (ca == d).all() and (cb == c).all()
+    q, s, _, _ = observables.replica_overlap([up, 1 - up, c], [1, 1, 1], [up, up, 1 - c], [1, 0, 1])
+    assert list(q) == [9, -9, -9] and s == [-9, 27, 243]
+    # chunked with carried states = whole; a chunk starting on a rejection uses the carried state
+    q1, s1, ca, cb = observables.replica_overlap([up, 1 - up], [1, 1], [up, up], [1, 0])
+    q2, s2, ca, cb = observables.replica_overlap([c], [1], [1 - c], [1], ca, cb)
+    assert list(q1) + list(q2) == list(q) and [x + y for x, y in zip(s1, s2)] == s
+    q3, s3, _, _ = observables.replica_overlap([c], [0], [c], [0], cur_a=up, cur_b=1 - up)
+    assert list(q3) == [-9] and s3 == [-9, 9, 81]
+
+
+def test_overlap_symmetries():
+    rng = np.random.default_rng(5)
+    a = rng.integers(0, 2, size=(7, 6, 6)); b = rng.integers(0, 2, size=(7, 6, 6))
+    q = observables.overlap(a, b)
+    assert (q == observables.overlap(b, a)).all()                              # symmetric
+    assert (observables.overlap(1 - a, b) == -q).all()                         # global flip of one replica
+    assert (observables.overlap(1 - a, 1 - b) == q).all()                      # Z2 symmetry of the pair
+    assert (q == 36 - 2 * (a != b).sum(axis=(1, 2))).all()                     # N - 2 Hamming distance
+    assert (np.abs(q) <= 36).all() and ((q - 36) % 2 == 0).all()
+
+
+def test_exact_chi_replicas_reproduce_boltzmann_overlap():
+    """two independent exact samplers of the same disorder: <q^2> -> sum_{s,s'} P(s) P(s') (s.s')^2 (brute force)"""
+    L, chi, beta, n_s = 3, 8, 0.9, 5000
+    Jr, Jd = make_couplings(L, 1, 78)
+    Jr, Jd = Jr[0], Jd[0]
+    cfgs, E_all, logZ, Pb = exact.brute_force(Jr, Jd, beta)
+    S = (2 * cfgs.reshape(len(cfgs), -1).astype(np.int64) - 1)
+    Q = S @ S.T
+    q2_exact = float(Pb @ (Q ** 2) @ Pb)
+    q4_exact = float(Pb @ (Q.astype(float) ** 4) @ Pb)
+    cache, _ = bmps.build_cache(Jr, Jd, beta, chi)
+    chains = []
+    for seed in (31, 32):
+        u = np.empty((n_s, L, L))
+        for r in range(L):
+            for c in range(L):
+                u[:, r, c] = philox.spin_uniforms(seed, 0, np.arange(n_s), r * L + c)
+        cfg, logq, _ = sampler.sample(cache, Jd, beta, u)
+        E = exact.energy(cfg, Jr, Jd)
+        acc, n_acc, *_ = metropolis.metropolis_scan(E, logq, beta, philox.metropolis_uniforms(seed, 0, np.arange(n_s)))
+        assert n_acc >= n_s - 3
+        chains.append((cfg, acc))
+    q, s, _, _ = observables.replica_overlap(chains[0][0], chains[0][1], chains[1][0], chains[1][1])
+    sigma = np.sqrt(max(q4_exact - q2_exact ** 2, 1e-12) / n_s)
+    assert abs(s[2] / n_s - q2_exact) < 4.5 * sigma
+    assert abs(s[0] / n_s) < 4.5 * np.sqrt(q2_exact / n_s)                     # <q> = 0 by the Z2 symmetry
