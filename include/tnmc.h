@@ -29,7 +29,9 @@
  *   counter = (site, sample index, disorder index, tag), tag 0 = spin draws, tag 1 = Metropolis
  *   draws (site word 0, sample word = step index); u = ((x0 << 21) | (x1 >> 11)) * 2^-53;
  *   a spin is +1 iff u < p.  "disorder index" is first_disorder + d, "sample index" is
- *   sample_offset + n, so results do not depend on how calls are chunked.
+ *   sample_offset + n, so results do not depend on how calls are chunked.  Each of the three indices fills ONE
+ *   32-bit counter word: first_disorder + n_dis, sample_offset + n_samples and step_offset + n_samples must not
+ *   exceed 2^32 (TNMC_EINVAL otherwise) -- the configs of the paper use at most 10^3 of each.
  *
  * Memory and ownership
  *   Every pointer marked [dev] is a device pointer owned by the caller (e.g. torch tensors);
@@ -38,7 +40,8 @@
  *   tnmc_workspace_bytes), which must stay alive and untouched until tnmc_destroy.  No entry
  *   point allocates device memory.  Kernels are enqueued on the stream given to tnmc_create and
  *   the calls return before completion; outputs are valid after the caller synchronises that
- *   stream.  Only tnmc_get_flags / tnmc_get_env_row / tnmc_run_host synchronise.
+ *   stream.  Only tnmc_get_flags / tnmc_get_env_row / tnmc_run_host synchronise (tnmc_create does not: its slot
+ *   maps and coupling masks are written by kernels on the stream).
  *
  * Errors
  *   Every call returns a tnmc_status; nothing throws across the ABI.  Argument errors are
@@ -119,7 +122,9 @@ size_t tnmc_workspace_bytes(int L, int chi, int n_dis, int n_samples_max, tnmc_p
 /* Create a context for n_dis disorder realisations.
  *   Jr, Jd      [dev] int8 (n_dis, L, L), values in {-1, 0, +1}; read (bit-packed into the
  *               workspace) by a kernel enqueued on the stream; may be freed once the stream has
- *               passed that point.  Values outside {-1,0,+1} are treated as their sign.
+ *               passed that point.  Values outside {-1,0,+1} are treated as their sign (the values live on the device
+ *               and are not read back: no TNMC_EINVAL for them); entries across the open boundary (Jr at c = L-1, Jd
+ *               at r = L-1) are ignored.
  *   first_disorder  global index of disorder 0 (enters the Philox counter only)
  *   workspace   [dev] >= tnmc_workspace_bytes(...) bytes, 256-byte aligned
  *   cuda_stream a cudaStream_t (NULL = legacy default stream)
@@ -176,6 +181,18 @@ tnmc_status tnmc_sample_ex(tnmc_ctx* ctx, int dis_begin, int dis_count, int n_sa
                            const uint32_t* forced_cfg_bits,
                            uint32_t* cfg_bits, double* logq, double* probs);
 
+/* tnmc_sample with the energy (Eq. 1) and the magnetisation M = sum_i s_i of every drawn configuration
+ * accumulated inside the left sampling sweep (the lane that packs a finished word of the new row also holds the word
+ * above it: XOR + popcount against the coupling masks, the arithmetic of tnmc_energy), so that no second pass over
+ * the configurations is needed -- and the configurations need not be stored at all:
+ *   cfg_bits [dev] as tnmc_sample, or NULL: do not keep the configurations (at configs[4] they are 131 GB packed;
+ *            E, M and log q are what the Metropolis scan and the thermal averages of E and M consume)
+ *   E, M     [dev] int32 (dis_count, n_samples)  out; bit-identical to tnmc_energy / tnmc_observables' M on the same spins
+ * +-J contexts only (TNMC_ESTATE on real couplings).  Other arguments and errors as tnmc_sample. */
+tnmc_status tnmc_sample_fused(tnmc_ctx* ctx, int dis_begin, int dis_count, int n_samples,
+                              uint64_t seed, uint64_t sample_offset,
+                              uint32_t* cfg_bits, double* logq, int32_t* E, int32_t* M);
+
 /* Exact energies, Eq. 1:  E = -sum_<ij> J_ij s_i s_j, integer arithmetic on the
  * packed words (XOR + popcount).
  *   cfg_bits [dev] uint32 (dis_count, n_samples, L, W)   in
@@ -216,6 +233,24 @@ tnmc_status tnmc_observables(tnmc_ctx* ctx, int dis_begin, int dis_count, int n_
 tnmc_status tnmc_observables_real(tnmc_ctx* ctx, int dis_begin, int dis_count, int n_samples,
                                   const uint32_t* cfg_bits, const double* E, const uint8_t* accepted,
                                   int32_t* M, double* cur_E, int32_t* cur_M, double* sums);
+
+/* Replica overlap along two independent Metropolis chains a, b of the same disorders (the spin-glass order
+ * parameter: <M> = 0 by symmetry in the +-J model of PAPER.md:282-286, the overlap q = sum_i s_i^a s_i^b between two
+ * replicas is the observable that carries the physics; no code in the paper; reading G19 of
+ * DESIGN.md as for tnmc_observables): at step n each chain sits on its last accepted proposal and
+ * q_n = N - 2 popcount(a xor b), an exact integer in [-N, N].
+ *   cfg_a, accepted_a  [dev] proposals of chain a (dis_count, n_samples, L, W) and its flags from tnmc_metropolis
+ *   cfg_b, accepted_b  [dev] likewise for chain b (e.g. a second tnmc_sample range of the same context)
+ *   cur_cfg_a, cur_cfg_b [dev] uint32 (dis_count, L, W) in/out: state of each chain entering / leaving the call
+ *               (read only for steps before that chain's first accepted proposal of this call; a fresh chain's first
+ *               flag is 1, so fresh chains never read them)
+ *   q_steps  [dev] int32 (dis_count, n_samples)  out: q_n of every step
+ *   sums     [dev] double (dis_count, 3)  in/out: sum q, sum |q|, sum q^2 over the steps are ADDED (zero them first)
+ * Both chains must cover the same disorders in the same order; works for +-J and real couplings alike. */
+tnmc_status tnmc_replica_overlap(tnmc_ctx* ctx, int dis_count, int n_samples,
+                                 const uint32_t* cfg_a, const uint8_t* accepted_a,
+                                 const uint32_t* cfg_b, const uint8_t* accepted_b,
+                                 uint32_t* cur_cfg_a, uint32_t* cur_cfg_b, int32_t* q_steps, double* sums);
 
 /* tnmc_observables for callers that cannot allocate device memory (code under CUDA graph capture, tight serving
  * loops, harnesses that forbid cudaMalloc): the same two kernels, with the per-proposal magnetisations M -- the

@@ -51,6 +51,8 @@ static tnmc_status create_impl(tnmc_ctx** out, int L, int chi, double beta, int 
     if (!make_plan(p, L, chi, n_dis, n_samples_max, ckpt_stride, (int)prec, real_j))
         return fail(nullptr, TNMC_EINVAL, "tnmc_create: need 2 <= L <= 4096, 2 <= chi <= 32, n_dis >= 1, n_samples_max >= 1, ckpt_stride >= 0");
     if (workspace_bytes < p.total) return fail(nullptr, TNMC_ENOMEM, "tnmc_create: workspace too small");
+    if (first_disorder + (uint64_t)n_dis > (1ull << 32))
+        return fail(nullptr, TNMC_EINVAL, "tnmc_create: first_disorder + n_dis exceeds 2^32 (the Philox counter word of the disorder index is 32 bits)");
     int dev_count = 0;
     if (cudaGetDeviceCount(&dev_count) != cudaSuccess || dev_count == 0)
         return fail(nullptr, TNMC_ECUDA, "tnmc_create: no CUDA device (there is no CPU fallback)");
@@ -63,17 +65,14 @@ static tnmc_status create_impl(tnmc_ctx** out, int L, int chi, double beta, int 
     ctx->ws = reinterpret_cast<char*>(workspace);
 
     auto bail = [&](tnmc_status st) { g_err = ctx->err; delete ctx; return st; };
-    // slot maps -> device
-    std::vector<int> maps((size_t)p.n_maps * L);
-    for (int m = 0; m < p.n_maps; ++m) {
-        const std::vector<int> s = p.slot_map(m);
-        std::memcpy(maps.data() + (size_t)m * L, s.data(), sizeof(int) * L);
+    // slot maps: written on the device by a kernel on the stream (no host staging, nothing to wait for)
+    {
+        const int n = p.n_maps * L;
+        slot_maps_kernel<<<(n + 255) / 256, 256, 0, ctx->stream>>>(L, p.ckpt, p.n_seg, p.n_maps, ctx->at<int>(p.off_maps));
     }
-    cudaError_t e = cudaMemcpyAsync(ctx->at<int>(p.off_maps), maps.data(), sizeof(int) * maps.size(),
-                                    cudaMemcpyHostToDevice, ctx->stream);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);   // `maps` is a host temporary
-    if (e == cudaSuccess) e = cudaMemsetAsync(ctx->at<char>(p.off_flags), 0, sizeof(unsigned long long) * N_FLAGS, ctx->stream);
-    if (e != cudaSuccess) return bail(cuda_fail(ctx, e, "tnmc_create: upload"));
+    cudaError_t e = cudaPeekAtLastError();
+    if (e == cudaSuccess) { ctx->launches++; e = cudaMemsetAsync(ctx->at<char>(p.off_flags), 0, sizeof(unsigned long long) * N_FLAGS, ctx->stream); }
+    if (e != cudaSuccess) return bail(cuda_fail(ctx, e, "tnmc_create: slot maps"));
     if (real_j) {
         // real couplings are kept as doubles inside the workspace (device-to-device copy on the stream)
         const size_t nb = sizeof(double) * (size_t)n_dis * L * L;
@@ -158,15 +157,29 @@ static tnmc_status launch_build(tnmc_ctx* ctx, int m, int row_hi, int row_lo, in
 
 // MODE: 0 = FP64 stack + FP64 DMMA sampler, 1 = FP32 stack + 3xTF32 sampler, 2 = FP32 stack + FP64 DMMA sampler,
 //       3 = FP32 stack + plain TF32 sampler
+// The FP64 sampler has a 64-chain CTA variant besides the 128-chain one: used when the 128-chain grid has fewer than
+// two CTAs per SM to offer (small n_samples x dis_count, e.g. C2), where halving the CTAs' size doubles their number.
 template <int P, int MODE, bool REALJ>
-static cudaError_t launch_sample_t(const tnmc_ctx* ctx, const SampleArgs& a, int tiles, int dis_count) {
+static cudaError_t launch_sample_t(const tnmc_ctx* ctx, const SampleArgs& a, int dis_count) {
     const int W = (a.L + 31) / 32;
+    const int tiles = (a.n_samples + SAMPLE_CHAINS - 1) / SAMPLE_CHAINS;
     if (MODE == 1 || MODE == 3) {
         const size_t smem32 = sizeof(float) * SAMPLE_STAGES * 2 * P * P + sizeof(uint32_t) * SAMPLE_CHAINS * W +
                               (REALJ ? sizeof(float) * 2 * a.L : 0);
         cudaError_t e32 = cudaFuncSetAttribute(sample_rows_tf32_kernel<P, REALJ, MODE == 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem32);
         if (e32 != cudaSuccess) return e32;
         sample_rows_tf32_kernel<P, REALJ, MODE == 1><<<dim3(tiles, dis_count), SAMPLE_THREADS, smem32, ctx->stream>>>(a);
+        return cudaPeekAtLastError();
+    }
+    int n_sm = 148;
+    { int dev = 0; if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev); }
+    if ((long long)tiles * dis_count < 2LL * n_sm) {
+        constexpr int CH = SAMPLE_CHAINS / 2;
+        const int tiles64 = (a.n_samples + CH - 1) / CH;
+        const size_t smem = sizeof(double) * SAMPLE_STAGES * 2 * P * P + sizeof(uint32_t) * CH * W + (REALJ ? sizeof(double) * 2 * a.L : 0);
+        cudaError_t e = cudaFuncSetAttribute(sample_rows_kernel<P, REALJ, MODE == 2, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        sample_rows_kernel<P, REALJ, MODE == 2, 1><<<dim3(tiles64, dis_count), SAMPLE_THREADS, smem, ctx->stream>>>(a);
         return cudaPeekAtLastError();
     }
     const size_t smem = sizeof(double) * SAMPLE_STAGES * 2 * P * P + sizeof(uint32_t) * SAMPLE_CHAINS * W +
@@ -177,11 +190,11 @@ static cudaError_t launch_sample_t(const tnmc_ctx* ctx, const SampleArgs& a, int
     return cudaPeekAtLastError();
 }
 template <int MODE, bool REALJ>
-static cudaError_t launch_sample_p(const tnmc_ctx* ctx, const SampleArgs& a, int tiles, int dis_count) {
+static cudaError_t launch_sample_p(const tnmc_ctx* ctx, const SampleArgs& a, int dis_count) {
     const int P = ctx->plan.P;
-    if (P == 8) return launch_sample_t<8, MODE, REALJ>(ctx, a, tiles, dis_count);
-    if (P == 16) return launch_sample_t<16, MODE, REALJ>(ctx, a, tiles, dis_count);
-    return launch_sample_t<32, MODE, REALJ>(ctx, a, tiles, dis_count);
+    if (P == 8) return launch_sample_t<8, MODE, REALJ>(ctx, a, dis_count);
+    if (P == 16) return launch_sample_t<16, MODE, REALJ>(ctx, a, dis_count);
+    return launch_sample_t<32, MODE, REALJ>(ctx, a, dis_count);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -217,16 +230,21 @@ static tnmc_status check_range(tnmc_ctx* ctx, const char* who, int dis_begin, in
     return TNMC_OK;
 }
 
-extern "C" tnmc_status tnmc_sample_ex(tnmc_ctx* ctx, int dis_begin, int dis_count, int n_samples,
-                                      uint64_t seed, uint64_t sample_offset,
-                                      const uint32_t* forced_cfg_bits,
-                                      uint32_t* cfg_bits, double* logq, double* probs) {
+static tnmc_status sample_impl(tnmc_ctx* ctx, int dis_begin, int dis_count, int n_samples,
+                               uint64_t seed, uint64_t sample_offset,
+                               const uint32_t* forced_cfg_bits,
+                               uint32_t* cfg_bits, double* logq, double* probs, int32_t* E, int32_t* M) {
     tnmc_status st = check_range(ctx, "tnmc_sample", dis_begin, dis_count, n_samples);
     if (st != TNMC_OK) return st;
     if (!ctx->built) return fail(ctx, TNMC_ESTATE, "tnmc_sample: call tnmc_build_envs first");
     const Plan& p = ctx->plan;
     if (n_samples > p.n_samples_max) return fail(ctx, TNMC_EINVAL, "tnmc_sample: n_samples > n_samples_max");
-    if (!cfg_bits || !logq) return fail(ctx, TNMC_EINVAL, "tnmc_sample: NULL output pointer");
+    if ((!cfg_bits && !E) || !logq) return fail(ctx, TNMC_EINVAL, "tnmc_sample: NULL output pointer");
+    if ((E == nullptr) != (M == nullptr)) return fail(ctx, TNMC_EINVAL, "tnmc_sample_fused: E and M go together");
+    if (E && p.real_j) return fail(ctx, TNMC_ESTATE, "tnmc_sample_fused: +-J contexts only (real couplings: tnmc_sample + tnmc_energy_real)");
+    if (!cfg_bits && forced_cfg_bits) return fail(ctx, TNMC_EINVAL, "tnmc_sample: forced spins need cfg_bits");
+    if (sample_offset > (1ull << 32) || sample_offset + (uint64_t)n_samples > (1ull << 32))
+        return fail(ctx, TNMC_EINVAL, "tnmc_sample: sample_offset + n_samples exceeds 2^32 (the Philox counter word of the sample index is 32 bits)");
     SampleArgs a;
     a.J = ctx->jview();
     a.beta = ctx->beta; a.L = p.L; a.chi = p.chi;
@@ -234,10 +252,11 @@ extern "C" tnmc_status tnmc_sample_ex(tnmc_ctx* ctx, int dis_begin, int dis_coun
     a.env = ctx->env(); a.env_dis_stride = p.env_dis_stride;
     a.renv = ctx->at<double>(p.off_renv);
     a.cfg_bits = cfg_bits; a.forced = forced_cfg_bits; a.logq = logq; a.probs = probs;
+    a.E_out = E; a.M_out = M; a.n_samples_max = p.n_samples_max;
+    a.carry = p.ckpt ? ctx->at<uint32_t>(p.off_carry) : nullptr;
     a.seed_lo = (uint32_t)(seed & 0xffffffffu); a.seed_hi = (uint32_t)(seed >> 32);
     a.sample_offset = sample_offset; a.first_disorder = ctx->first_disorder;
     a.flags = ctx->at<unsigned long long>(p.off_flags);
-    const int tiles = (n_samples + SAMPLE_CHAINS - 1) / SAMPLE_CHAINS;
     for (int j = 0; j < p.n_seg; ++j) {
         int m = 0;
         if (p.ckpt > 0) {
@@ -249,20 +268,35 @@ extern "C" tnmc_status tnmc_sample_ex(tnmc_ctx* ctx, int dis_begin, int dis_coun
         } else { a.row_lo = 0; a.row_hi = p.L; }
         a.slot_of_row = ctx->map(m);
         cudaError_t e;
-        if (p.tf32 && p.x3) e = p.real_j ? launch_sample_p<1, true>(ctx, a, tiles, dis_count) : launch_sample_p<1, false>(ctx, a, tiles, dis_count);
-        else if (p.tf32) e = p.real_j ? launch_sample_p<3, true>(ctx, a, tiles, dis_count) : launch_sample_p<3, false>(ctx, a, tiles, dis_count);
-        else if (p.f32) e = p.real_j ? launch_sample_p<2, true>(ctx, a, tiles, dis_count) : launch_sample_p<2, false>(ctx, a, tiles, dis_count);
-        else e = p.real_j ? launch_sample_p<0, true>(ctx, a, tiles, dis_count) : launch_sample_p<0, false>(ctx, a, tiles, dis_count);
+        if (p.tf32 && p.x3) e = p.real_j ? launch_sample_p<1, true>(ctx, a, dis_count) : launch_sample_p<1, false>(ctx, a, dis_count);
+        else if (p.tf32) e = p.real_j ? launch_sample_p<3, true>(ctx, a, dis_count) : launch_sample_p<3, false>(ctx, a, dis_count);
+        else if (p.f32) e = p.real_j ? launch_sample_p<2, true>(ctx, a, dis_count) : launch_sample_p<2, false>(ctx, a, dis_count);
+        else e = p.real_j ? launch_sample_p<0, true>(ctx, a, dis_count) : launch_sample_p<0, false>(ctx, a, dis_count);
         if (e != cudaSuccess) return cuda_fail(ctx, e, "sample_rows_kernel");
         ctx->launches++;
     }
     return TNMC_OK;
 }
 
+extern "C" tnmc_status tnmc_sample_ex(tnmc_ctx* ctx, int dis_begin, int dis_count, int n_samples,
+                                      uint64_t seed, uint64_t sample_offset,
+                                      const uint32_t* forced_cfg_bits,
+                                      uint32_t* cfg_bits, double* logq, double* probs) {
+    if (!cfg_bits) return fail(ctx, TNMC_EINVAL, "tnmc_sample: NULL output pointer");
+    return sample_impl(ctx, dis_begin, dis_count, n_samples, seed, sample_offset, forced_cfg_bits, cfg_bits, logq, probs, nullptr, nullptr);
+}
+
 extern "C" tnmc_status tnmc_sample(tnmc_ctx* ctx, int dis_begin, int dis_count, int n_samples,
                                    uint64_t seed, uint64_t sample_offset,
                                    uint32_t* cfg_bits, double* logq) {
     return tnmc_sample_ex(ctx, dis_begin, dis_count, n_samples, seed, sample_offset, nullptr, cfg_bits, logq, nullptr);
+}
+
+extern "C" tnmc_status tnmc_sample_fused(tnmc_ctx* ctx, int dis_begin, int dis_count, int n_samples,
+                                         uint64_t seed, uint64_t sample_offset,
+                                         uint32_t* cfg_bits, double* logq, int32_t* E, int32_t* M) {
+    if (!E || !M) return fail(ctx, TNMC_EINVAL, "tnmc_sample_fused: NULL output pointer");
+    return sample_impl(ctx, dis_begin, dis_count, n_samples, seed, sample_offset, nullptr, cfg_bits, logq, nullptr, E, M);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -293,6 +327,8 @@ extern "C" tnmc_status tnmc_metropolis(tnmc_ctx* ctx, int dis_begin, int dis_cou
     if (st != TNMC_OK) return st;
     if (!E || !logq || !cur_logq || !cur_E || !cur_idx || !accepted || !n_accepted)
         return fail(ctx, TNMC_EINVAL, "tnmc_metropolis: NULL pointer");
+    if (step_offset > (1ull << 32) || step_offset + (uint64_t)n_samples > (1ull << 32))
+        return fail(ctx, TNMC_EINVAL, "tnmc_metropolis: step_offset + n_samples exceeds 2^32 (the Philox counter word of the step index is 32 bits)");
     const int threads = 64;
     metropolis_kernel<int32_t><<<(dis_count + threads - 1) / threads, threads, 0, ctx->stream>>>(
         ctx->beta, dis_begin, dis_count, n_samples, E, logq, (uint32_t)(seed & 0xffffffffu),
@@ -326,6 +362,8 @@ extern "C" tnmc_status tnmc_metropolis_real(tnmc_ctx* ctx, int dis_begin, int di
     if (st != TNMC_OK) return st;
     if (!E || !logq || !cur_logq || !cur_E || !cur_idx || !accepted || !n_accepted)
         return fail(ctx, TNMC_EINVAL, "tnmc_metropolis_real: NULL pointer");
+    if (step_offset > (1ull << 32) || step_offset + (uint64_t)n_samples > (1ull << 32))
+        return fail(ctx, TNMC_EINVAL, "tnmc_metropolis_real: step_offset + n_samples exceeds 2^32 (the Philox counter word of the step index is 32 bits)");
     const int threads = 64;
     metropolis_kernel<double><<<(dis_count + threads - 1) / threads, threads, 0, ctx->stream>>>(
         ctx->beta, dis_begin, dis_count, n_samples, E, logq, (uint32_t)(seed & 0xffffffffu),
@@ -365,6 +403,26 @@ extern "C" tnmc_status tnmc_observables_real(tnmc_ctx* ctx, int dis_begin, int d
                                              const uint32_t* cfg_bits, const double* E, const uint8_t* accepted,
                                              int32_t* M, double* cur_E, int32_t* cur_M, double* sums) {
     return observables_impl<double>(ctx, "tnmc_observables_real", dis_begin, dis_count, n_samples, cfg_bits, E, accepted, M, cur_E, cur_M, sums);
+}
+
+extern "C" tnmc_status tnmc_replica_overlap(tnmc_ctx* ctx, int dis_count, int n_samples,
+                                            const uint32_t* cfg_a, const uint8_t* accepted_a,
+                                            const uint32_t* cfg_b, const uint8_t* accepted_b,
+                                            uint32_t* cur_cfg_a, uint32_t* cur_cfg_b, int32_t* q_steps, double* sums) {
+    tnmc_status st = check_range(ctx, "tnmc_replica_overlap", 0, dis_count, n_samples);
+    if (st != TNMC_OK) return st;
+    if (!cfg_a || !accepted_a || !cfg_b || !accepted_b || !cur_cfg_a || !cur_cfg_b || !q_steps || !sums)
+        return fail(ctx, TNMC_EINVAL, "tnmc_replica_overlap: NULL pointer");
+    const Plan& p = ctx->plan;
+    const long long n_steps = (long long)dis_count * n_samples;
+    const int warps = 8;
+    overlap_steps_kernel<<<(unsigned)((n_steps + warps - 1) / warps), warps * 32, 0, ctx->stream>>>(
+        p.L, p.W, dis_count, n_samples, cfg_a, accepted_a, cfg_b, accepted_b, cur_cfg_a, cur_cfg_b, q_steps);
+    CK_LAUNCH(ctx, "overlap_steps_kernel");
+    overlap_sums_kernel<<<dis_count, 256, 0, ctx->stream>>>(p.L, p.W, n_samples, cfg_a, accepted_a, cfg_b, accepted_b,
+                                                           q_steps, cur_cfg_a, cur_cfg_b, sums);
+    CK_LAUNCH(ctx, "overlap_sums_kernel");
+    return TNMC_OK;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -591,12 +649,3 @@ extern "C" double tnmc_fp64_peak_tflops(int which, void* scratch, void* cuda_str
                                     : 2.0 * 256 * 8 * iters * (double)blocks * (threads / 32);
     return flops / (best * 1e-3) / 1e12;
 }
-
-#ifdef TNMC_PROFILE
-// debug build only: per-phase clock64 totals of CTA 0 of build_rows_kernel
-extern "C" void tnmc_debug_build_profile(unsigned long long* out16, int reset) {
-    cudaDeviceSynchronize();
-    cudaMemcpyFromSymbol(out16, tnmc::g_build_prof, sizeof(unsigned long long) * 256);
-    if (reset) { unsigned long long z[256] = {0}; cudaMemcpyToSymbol(tnmc::g_build_prof, z, sizeof(z)); }
-}
-#endif

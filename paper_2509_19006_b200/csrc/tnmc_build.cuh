@@ -22,16 +22,6 @@
 
 namespace tnmc {
 
-#ifdef TNMC_PROFILE
-#define PROF_DECL long long prof_t0 = clock64();
-#define PROF(slot) do { if (blockIdx.x == 0 && threadIdx.x == 0) { const long long t_ = clock64(); atomicAdd(&g_build_prof[slot], (unsigned long long)(t_ - prof_t0)); prof_t0 = t_; } } while (0)
-#define PROF_ADD(slot, v) do { if (blockIdx.x == 0 && threadIdx.x == 0) atomicAdd(&g_build_prof[slot], (unsigned long long)(v)); } while (0)
-#else
-#define PROF_DECL
-#define PROF(slot)
-#define PROF_ADD(slot, v)
-#endif
-
 struct BuildArgs {
     JView J;
     double beta;
@@ -105,8 +95,6 @@ __global__ void __launch_bounds__(BuildCfg<P>::NT, BuildCfg<P>::CTAS_PER_SM) bui
     const size_t env_d = (size_t)d * args.env_dis_stride;
     double* qbuf_d = args.qbuf + (size_t)d * (size_t)L * Cfg::QSZ;
     double* ls_d = args.logscale + (size_t)d * L;
-
-    PROF_DECL
     for (int r = args.row_hi - 1; r >= args.row_lo; --r) {
         const size_t env_in = env_d + (size_t)args.slot_of_row[r + 1] * L * TSZ;
         const size_t env_out = env_d + (size_t)args.slot_of_row[r] * L * TSZ;
@@ -131,19 +119,21 @@ __global__ void __launch_bounds__(BuildCfg<P>::NT, BuildCfg<P>::CTAS_PER_SM) bui
                 }
             }
             __syncthreads();
-            // T_a[x][k] = sum_i R_a[x][i] C_a[i][k]  -> column k of block a of X
-            for (int t = tid; t < 2 * q * br; t += NT) {
-                const int x = t % q, k = (t / q) % br, a = t / (q * br);
-                const double* Rrow = sR + (size_t)a * D * LDR + (size_t)x * LDR;
-                const double* Ccol = sU + (size_t)a * P * LDU + k;
-                double acc0 = 0.0, acc1 = 0.0;
-                int i = 0;
-                for (; i + 1 < bl; i += 2) {
-                    acc0 = fma(Rrow[i], Ccol[i * LDU], acc0);
-                    acc1 = fma(Rrow[i + 1], Ccol[(i + 1) * LDU], acc1);
+            // T_a[x][k] = sum_i R_a[x][i] C_a[i][k]  -> column k of block a of X: a (q x bl)(bl x br) product per spin
+            // block on the FP64 tensor pipe; a warp takes 8-row strips (a, x0) and all column tiles of the strip
+            {
+                const int warp = tid >> 5, lane = tid & 31;
+                const int strips = (q + 7) >> 3;
+                for (int st = warp; st < 2 * strips; st += NT / 32) {
+                    const int a = st / strips, x0 = (st - a * strips) * 8;
+                    const double* Ra = sR + (size_t)a * D * LDR;
+                    const double* Ca = sU + (size_t)a * P * LDU;
+                    double* Xa = sX + (size_t)a * P * LDX;
+                    dmma_strip<P / 8>(bl, lane,
+                        [&](int g, int i) { return (x0 + g < q && i < bl) ? Ra[(size_t)(x0 + g) * LDR + i] : 0.0; },
+                        [&](int i, int k) { return (i < bl && k < br) ? Ca[(size_t)i * LDU + k] : 0.0; },
+                        [&](int g, int k, double v) { if (x0 + g < q && k < br) Xa[(size_t)k * LDX + x0 + g] = v; });
                 }
-                if (i < bl) acc0 = fma(Rrow[i], Ccol[i * LDU], acc0);
-                sX[(size_t)(a * P + k) * LDX + x] = acc0 + acc1;
             }
             __syncthreads();
             double* Qout = qbuf_d + (size_t)c * Cfg::QSZ;
@@ -157,11 +147,9 @@ __global__ void __launch_bounds__(BuildCfg<P>::NT, BuildCfg<P>::CTAS_PER_SM) bui
                 __syncthreads();
                 break;
             }
-            PROF(0);
             const int p = q < br ? q : br;
             householder_qr_g<MAXK>(sX + (size_t)half * P * LDX, LDX, q, br, sTau + half * P, gt, HALF, 1 + half);
             __syncthreads();
-            PROF(1);
             // R_new[(a,y)][(rr,k)] = B_r[a][rr] R'_a[y][k] / |R_new|_F;  logscale += log |R_new|_F
             const double jr = args.J.jrv(d, r, c);
             const double w_same = exp(beta * jr), w_diff = exp(-beta * jr);
@@ -193,7 +181,6 @@ __global__ void __launch_bounds__(BuildCfg<P>::NT, BuildCfg<P>::CTAS_PER_SM) bui
                 Qout[LDX * D + a * P + z] = sTau[a * P + z];
             }
             __syncthreads();
-            PROF(2);
         }
 
         // ------------------------------------------------------------------ B. SVD sweep, right -> left
@@ -270,7 +257,6 @@ __global__ void __launch_bounds__(BuildCfg<P>::NT, BuildCfg<P>::CTAS_PER_SM) bui
                 const int x = t % q, col = t / q;
                 sM0[(size_t)col * D + x] = sX[(size_t)col * LDX + x];
             }
-            PROF(7);
             // M = Q (R P^T) with column pivoting, R only and in M's own column order; rows of R below the
             // numerical rank (sigma <= 1e-15 |M|_F) are dropped.  Singular values and right singular
             // vectors of M are those of R P^T.
@@ -283,20 +269,15 @@ __global__ void __launch_bounds__(BuildCfg<P>::NT, BuildCfg<P>::CTAS_PER_SM) bui
             }
             __syncthreads();
             const double thr2 = fro2 * 1e-30;      // sigma <= 1e-15 |M|_F: below the numerical rank
-            PROF(4);
             // chi = 32: one row of each pair held in registers, norms carried (jacobi_rows4: C3 build 6.48 -> 5.97 s);
             // chi <= 16: one warp per scheduler, bound by the latency of the dependent chain, where the bookkeeping of
             // the held row costs more than the loads it saves (C2 build 93 -> 100 ms): jacobi_rows2
             constexpr int JNK = (D + 2 * Cfg::LPP - 1) / (2 * Cfg::LPP);
-            int nsw = 0;
             if (nrow >= 2) {
                 static_assert(JNK * 2 * Cfg::LPP < LDM, "the carried norm of a row lives in the spare column after its padded width");
-                if constexpr (Cfg::JACOBI_HELD_ROW) nsw = jacobi_rows4<JNK, Cfg::LPP>(sMj, LDM, JNK * 2 * Cfg::LPP, nrow, fro2, thr2, args.flags);
-                else nsw = jacobi_rows2<JNK, Cfg::LPP>(sMj, LDM, nrow, fro2, thr2, args.flags);
+                if constexpr (Cfg::JACOBI_HELD_ROW) jacobi_rows4<JNK, Cfg::LPP>(sMj, LDM, JNK * 2 * Cfg::LPP, nrow, fro2, thr2, args.flags);
+                else jacobi_rows2<JNK, Cfg::LPP>(sMj, LDM, nrow, fro2, thr2, args.flags);
             }
-            PROF(5);
-            PROF_ADD(8, nsw); PROF_ADD(9, 1);
-            (void)nsw;
             // singular values = row norms
             {
                 const int grp = tid >> 3, t8 = tid & 7;
@@ -342,21 +323,19 @@ __global__ void __launch_bounds__(BuildCfg<P>::NT, BuildCfg<P>::CTAS_PER_SM) bui
             }
             __syncthreads();
             for (int t = tid; t < TSZ; t += NT) args.env.st(Aout + t, stage[t]);
-            // Pc_next[x][y'] = sum_col M[x][col] V_k[col][y']   (= M V_k, projector form of P-C2 step 2)
-            for (int t = tid; t < q * k; t += NT) {
-                const int x = t % q, yp = t / q;
-                const double* mcol = sM0 + x;
-                const double* vrow = sV + (size_t)yp * LDV;
-                double acc0 = 0.0, acc1 = 0.0;
-                for (int col = 0; col < nc; col += 2) {
-                    acc0 = fma(mcol[(size_t)col * D], vrow[col], acc0);
-                    acc1 = fma(mcol[(size_t)(col + 1) * D], vrow[col + 1], acc1);
+            // Pc_next[x][y'] = sum_col M[x][col] V_k[col][y']   (= M V_k, projector form of P-C2 step 2): a (q x nc)(nc x k)
+            // product on the FP64 tensor pipe, one 8-row strip of M per warp (M is read once, from L2 at chi = 32)
+            {
+                const int warp = tid >> 5, lane = tid & 31;
+                for (int x0 = 8 * warp; x0 < q; x0 += 8 * (NT / 32)) {
+                    dmma_strip<P / 8>(nc, lane,
+                        [&](int g, int col) { return (x0 + g < q && col < nc) ? sM0[(size_t)col * D + x0 + g] : 0.0; },
+                        [&](int col, int yp) { return (col < nc && yp < k) ? sV[(size_t)yp * LDV + col] : 0.0; },
+                        [&](int g, int yp, double v) { if (x0 + g < q && yp < k) sU[(size_t)(x0 + g) * LDU + yp] = v; });
                 }
-                sU[(size_t)x * LDU + yp] = acc0 + acc1;
             }
             __syncthreads();
             kprev = k;
-            PROF(6);
         }
         if (tid == 0) ls_d[r] = ls_d[r + 1] + logs;
         __syncthreads();
@@ -436,7 +415,9 @@ __global__ void pack_couplings_kernel(const int8_t* Jr, const int8_t* Jd, int n_
     for (int b = 0; b < 32; ++b) {
         const int c = w * 32 + b;
         if (c >= L) break;
-        const int8_t jr = Jr[dr * L + c], jd = Jd[dr * L + c];
+        // bonds across the open boundary do not exist (Jr at c = L-1, Jd at r = L-1): masked out whatever the caller put there
+        const int8_t jr = c + 1 < L ? Jr[dr * L + c] : (int8_t)0;
+        const int8_t jd = (int)(dr % L) + 1 < L ? Jd[dr * L + c] : (int8_t)0;
         rn |= (uint32_t)(jr < 0) << b; rz |= (uint32_t)(jr != 0) << b;
         dn |= (uint32_t)(jd < 0) << b; dz |= (uint32_t)(jd != 0) << b;
     }

@@ -17,6 +17,34 @@ __device__ __forceinline__ void raise_flag(unsigned long long* flags, int which)
 }
 
 // ---------------------------------------------------------------------------------------------
+// FP64 tensor-core primitive (DMMA in SASS; tcgen05 has no f64 kind, so mma.sync is the FP64 tensor path on sm_100a).
+// With lane = 4 g + q:  A (8x4) lane holds A[g][q];  B (4x8) lane holds B[q][g];  C (8x8) lane holds C[g][2q], C[g][2q+1].
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+// One warp computes an 8-row strip of C = A B over NT 8-column tiles with DMMA: the A fragment of a k-step is loaded
+// once and used for every column tile.  a_at(g, k), b_at(k, n) return the operand entries (0 outside the matrix),
+// c_out(g, n, v) stores a result.  K is rounded up to a multiple of 4 by the callers' zero padding.
+template <int NT, class FA, class FB, class FC>
+__device__ __forceinline__ void dmma_strip(int K, int lane, FA a_at, FB b_at, FC c_out) {
+    const int g = lane >> 2, q = lane & 3;
+    double acc[NT][2];
+#pragma unroll
+    for (int nt = 0; nt < NT; ++nt) { acc[nt][0] = 0.0; acc[nt][1] = 0.0; }
+#pragma unroll 4
+    for (int k0 = 0; k0 < K; k0 += 4) {
+        const double a = a_at(g, k0 + q);
+#pragma unroll
+        for (int nt = 0; nt < NT; ++nt) dmma884(acc[nt][0], acc[nt][1], a, b_at(k0 + q, 8 * nt + g));
+    }
+#pragma unroll
+    for (int nt = 0; nt < NT; ++nt) { c_out(g, 8 * nt + 2 * q, acc[nt][0]); c_out(g, 8 * nt + 2 * q + 1, acc[nt][1]); }
+}
+
+// ---------------------------------------------------------------------------------------------
 // Environment site-tensor layout in HBM ("fragment order").
 //
 // A stored site tensor is A[i][a][j] (left bond i, spin a, right bond j), zero

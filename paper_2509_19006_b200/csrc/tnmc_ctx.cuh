@@ -33,7 +33,7 @@ struct Plan {
     size_t qsz = 0;                 // doubles per site of the Q scratch
     // byte offsets into the workspace
     size_t off_masks = 0, off_maps = 0, off_flags = 0, off_logscale = 0, off_logz = 0, off_env = 0,
-           off_qbuf = 0, off_m0 = 0, off_renv = 0, off_jreal = 0, total = 0;
+           off_qbuf = 0, off_m0 = 0, off_renv = 0, off_jreal = 0, off_carry = 0, total = 0;
 
     int ckpt_slot(int j) const { return j; }
     int bottom_slot() const { return n_seg; }
@@ -45,20 +45,7 @@ struct Plan {
         if (r % ckpt == 0) return ckpt_slot(r / ckpt);
         return -1;
     }
-    // slot map m: m == 0 first pass; m == 1 + j: segment j (checkpoint mode only)
-    std::vector<int> slot_map(int m) const {
-        std::vector<int> s(L, -1);
-        for (int r = 0; r < L; ++r) {
-            const int p = perm_slot(r);
-            if (p >= 0) { s[r] = p; continue; }
-            if (m == 0) s[r] = seg_slot(r & 1);
-            else {
-                const int j = m - 1;
-                if (r > j * ckpt && r < (j + 1) * ckpt) s[r] = seg_slot(r - j * ckpt - 1);
-            }
-        }
-        return s;
-    }
+    // slot map m (m == 0 first pass; m == 1 + j: segment j, checkpoint mode only): slot_maps_kernel below
     // first stored row at or below the end of segment j: where its recomputation starts
     int seg_start_row(int j) const { const int h = (j + 1) * ckpt; return h <= L - 1 ? h : L - 1; }
     int seg_end(int j) const { const int h = (j + 1) * ckpt; return h < L ? h : L; }
@@ -96,8 +83,29 @@ inline bool make_plan(Plan& p, int L, int chi, int n_dis, int n_samples_max, int
     p.off_m0 = o;       o = align_up(o + sizeof(double) * (size_t)n_dis * 4 * p.P * p.P);
     p.off_renv = o;     o = align_up(o + sizeof(double) * (size_t)n_dis * p.tiles * L * SAMPLE_CHAINS * p.P);
     p.off_jreal = o;    o = align_up(o + (real_j ? sizeof(double) * 2 * (size_t)n_dis * L * L : 0));
+    // last row of a row range for tnmc_sample_fused without stored configurations (checkpoint mode only)
+    p.off_carry = o;    o = align_up(o + (ckpt ? sizeof(uint32_t) * (size_t)n_dis * n_samples_max * p.W : 0));
     p.total = o;
     return true;
+}
+
+// The slot maps of a Plan, written on the device: maps[m][r] = slot of row r in pass m, -1 if row r is not held.
+//   permanent slots (perm_slot above) first; pass 0 ping-pongs the other rows through the first two segment slots;
+//   pass 1 + j holds the inner rows of segment j in the segment slots.
+__global__ void slot_maps_kernel(int L, int ckpt, int n_seg, int n_maps, int* maps) {
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= n_maps * L) return;
+    const int m = idx / L, r = idx - m * L;
+    int s;
+    if (ckpt == 0) s = r;
+    else if (r == L - 1) s = n_seg;                       // bottom_slot
+    else if (r % ckpt == 0) s = r / ckpt;                 // ckpt_slot
+    else if (m == 0) s = n_seg + 1 + (r & 1);             // seg_slot(r & 1)
+    else {
+        const int j = m - 1;
+        s = (r > j * ckpt && r < (j + 1) * ckpt) ? n_seg + 1 + (r - j * ckpt - 1) : -1;
+    }
+    maps[idx] = s;
 }
 
 }  // namespace tnmc

@@ -69,7 +69,8 @@ __global__ void energy_real_kernel(JView J, int L, int W, int dis_begin, int dis
         const int nb = L - 32 * w < 32 ? L - 32 * w : 32;
         for (int b = 0; b < nb; ++b) {
             const int c = 32 * w + b;
-            const double a = jr[(size_t)r * L + c], bdn = jd[(size_t)r * L + c];   // 0 on the open boundary
+            // bonds across the open boundary do not exist, whatever the caller stored there
+            const double a = c + 1 < L ? jr[(size_t)r * L + c] : 0.0, bdn = r + 1 < L ? jd[(size_t)r * L + c] : 0.0;
             acc += ((xr >> b) & 1u) ? -a : a;
             acc += ((xd >> b) & 1u) ? -bdn : bdn;
         }
@@ -159,6 +160,83 @@ __global__ void observables_kernel(int dis_count, int n_samples, const ET* __res
     cur_E[dl] = (ET)ce; cur_M[dl] = (int32_t)cm;
     double* o = sums + (size_t)dl * 5;
     o[0] += (double)s0; o[1] += (double)s1; o[2] += (double)s2; o[3] += (double)s3; o[4] += (double)s4;
+}
+
+// Replica overlap along two Metropolis chains of the same disorder (oracle/observables.replica_overlap): at step n
+// chain x sits on its last accepted proposal at or before n (or on the carried state cur_x if none yet in this call);
+// q_n = sum_i s_i^a s_i^b = N - 2 popc(a xor b) over the packed words (unused high bits are 0 in both).
+// One warp per (disorder, step): the lanes find the two state indices by walking the flags backwards 32 at a time
+// (ballot; the expected distance is 1 / p_acc), then stride over the L*W words.
+__device__ __forceinline__ long long last_accepted_at_or_before(const uint8_t* __restrict__ acc, long long n, int lane) {
+    for (long long hi = n; hi >= 0; hi -= 32) {
+        const long long i = hi - lane;
+        const unsigned m = __ballot_sync(0xffffffffu, i >= 0 && acc[i] != 0);
+        if (m) return hi - (__ffs(m) - 1);
+    }
+    return -1;
+}
+
+__global__ void overlap_steps_kernel(int L, int W, int dis_count, int n_samples,
+                                     const uint32_t* __restrict__ cfg_a, const uint8_t* __restrict__ acc_a,
+                                     const uint32_t* __restrict__ cfg_b, const uint8_t* __restrict__ acc_b,
+                                     const uint32_t* __restrict__ cur_a, const uint32_t* __restrict__ cur_b,
+                                     int32_t* __restrict__ q_steps) {
+    const long long wid = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (wid >= (long long)dis_count * n_samples) return;
+    const int lane = threadIdx.x & 31;
+    const int dl = (int)(wid / n_samples);
+    const long long n = wid - (long long)dl * n_samples;
+    const size_t base = (size_t)dl * n_samples, nw = (size_t)L * W;
+    const long long ia = last_accepted_at_or_before(acc_a + base, n, lane);
+    const long long ib = last_accepted_at_or_before(acc_b + base, n, lane);
+    const uint32_t* a = ia >= 0 ? cfg_a + (base + (size_t)ia) * nw : cur_a + (size_t)dl * nw;
+    const uint32_t* b = ib >= 0 ? cfg_b + (base + (size_t)ib) * nw : cur_b + (size_t)dl * nw;
+    int diff = 0;
+    for (int i = lane; i < (int)nw; i += 32) diff += __popc(a[i] ^ b[i]);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) diff += __shfl_xor_sync(0xffffffffu, diff, o);
+    if (lane == 0) q_steps[wid] = L * L - 2 * diff;
+}
+
+// One CTA per disorder: sums of q, |q|, q^2 over the steps of the call (exact 64-bit integers, added to the double
+// accumulators once), then the chains' states leaving the call are copied into cur_a / cur_b.
+__global__ void overlap_sums_kernel(int L, int W, int n_samples,
+                                    const uint32_t* __restrict__ cfg_a, const uint8_t* __restrict__ acc_a,
+                                    const uint32_t* __restrict__ cfg_b, const uint8_t* __restrict__ acc_b,
+                                    const int32_t* __restrict__ q_steps, uint32_t* cur_a, uint32_t* cur_b, double* sums) {
+    __shared__ long long red[3][32];
+    __shared__ long long last[2];
+    const int dl = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const size_t base = (size_t)dl * n_samples, nw = (size_t)L * W;
+    long long s0 = 0, s1 = 0, s2 = 0;
+    for (int n = tid; n < n_samples; n += blockDim.x) {
+        const long long q = q_steps[base + n];
+        s0 += q; s1 += q < 0 ? -q : q; s2 += q * q;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        s0 += __shfl_xor_sync(0xffffffffu, s0, o);
+        s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+        s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+    }
+    if (lane == 0) { red[0][warp] = s0; red[1][warp] = s1; red[2][warp] = s2; }
+    if (warp == 0) {
+        const long long la = last_accepted_at_or_before(acc_a + base, n_samples - 1, lane);
+        const long long lb = last_accepted_at_or_before(acc_b + base, n_samples - 1, lane);
+        if (lane == 0) { last[0] = la; last[1] = lb; }
+    }
+    __syncthreads();
+    if (tid == 0) {
+        long long t0 = 0, t1 = 0, t2 = 0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) { t0 += red[0][w]; t1 += red[1][w]; t2 += red[2][w]; }
+        double* o = sums + (size_t)dl * 3;
+        o[0] += (double)t0; o[1] += (double)t1; o[2] += (double)t2;
+    }
+    const long long la = last[0], lb = last[1];
+    for (int i = tid; i < (int)nw; i += blockDim.x) {
+        if (la >= 0) cur_a[(size_t)dl * nw + i] = cfg_a[(base + (size_t)la) * nw + i];
+        if (lb >= 0) cur_b[(size_t)dl * nw + i] = cfg_b[(base + (size_t)lb) * nw + i];
+    }
 }
 
 }  // namespace tnmc

@@ -11,10 +11,6 @@
 
 namespace tnmc {
 
-#ifdef TNMC_PROFILE
-__device__ unsigned long long g_build_prof[256];   // debug build only
-#endif
-
 // block-wide sum of one double per thread; result valid in all threads. scratch: >= 32 doubles
 __device__ __forceinline__ double block_sum(double v, double* scratch) {
 #pragma unroll
@@ -378,7 +374,8 @@ __device__ double householder_qrcp2(double* X, int ld, int m, int n, double* cn,
 //   d = b - a, h = sqrt(d^2 + 4 g^2), u = |d| + h, w = 1 / sqrt(u^2 + 4 g^2), cos = u w, sin = sign(d) 2 g w.
 // The caller zero-pads every row to the full 2 LPP NK columns (rotations keep zeros zero).
 // All n rows take part (n even); rows at or below thr2 are left alone.  A sweep is the last one when every pair it
-// met had |cos| <= 1e-8 BEFORE its rotation (the rotation is still applied: quadratic convergence leaves ~1e-16).
+// met had |cos| <= 1e-6 BEFORE its rotation (the rotation is still applied: quadratic convergence leaves ~1e-12, two
+// orders below the 1e-10 the parity needs; 1e-8 measured the same deviations from the oracle on all of C2 and 2 % more time).
 // The test is purely relative: every kept row v enters M V_k V_k^T, so a row of tiny sigma that is left at an
 // angle eps from a dominant row changes the state by eps * sigma_1, whatever its own sigma.  (Round 1 also let a
 // sweep end when |g| <= 256 eps |M|_F max(|x|,|y|); on C2 beta = 2 -- kept sigma down to 1e-15 sigma_1 -- that left
@@ -392,7 +389,7 @@ __device__ int jacobi_rows2(double* M, int ld, int n, double fro2, double thr2, 
     (void)fro2;
     const unsigned gmask = ((1u << LPP) - 1u) << ((threadIdx.x & 31) & ~(LPP - 1));
     const double rot2 = 256.0 * 4.930380657631324e-32;             // (16 eps)^2
-    const double big2 = 1e-16;                                     // (1e-8)^2
+    const double big2 = 1e-12;                                     // (1e-6)^2
     const int c0 = 2 * t8;                                         // this lane's columns: c0 + 2 LPP k, c0 + 2 LPP k + 1
     int sweep = 0;
     for (; sweep < 60; ++sweep) {
@@ -482,7 +479,7 @@ __device__ int jacobi_rows4(double* M, int ld, int nslot, int n, double fro2, do
     (void)fro2;
     const unsigned gmask = ((1u << LPP) - 1u) << ((threadIdx.x & 31) & ~(LPP - 1));
     const double rot2 = 256.0 * 4.930380657631324e-32;             // (16 eps)^2
-    const double big2 = 1e-16;                                     // (1e-8)^2
+    const double big2 = 1e-12;                                     // (1e-6)^2
     const int c0 = 2 * t8;
     int sweep = 0;
     for (; sweep < 60; ++sweep) {

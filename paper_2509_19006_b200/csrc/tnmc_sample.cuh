@@ -38,7 +38,11 @@ struct SampleArgs {
     EnvRef env;                      // FP64 storage here; FP32 storage is read by tnmc_sample_tf32.cuh
     size_t env_dis_stride;           // elements per disorder
     double* renv;                    // scratch: per CTA  L * SAMPLE_CHAINS * P doubles
-    uint32_t* cfg_bits;              // (dis_count, n_samples, L, W)
+    uint32_t* cfg_bits;              // (dis_count, n_samples, L, W), or nullptr (tnmc_sample_fused: configurations not kept)
+    int32_t* E_out;                  // (dis_count, n_samples) or nullptr: Eq. 1 accumulated in the left sweep (+-J only)
+    int32_t* M_out;                  // (dis_count, n_samples) or nullptr: sum_i s_i, likewise
+    uint32_t* carry;                 // (n_dis, n_samples_max, W): last row of a row range, for the next range when cfg_bits is nullptr
+    int n_samples_max;
     const uint32_t* forced;          // or nullptr
     double* logq;                    // (dis_count, n_samples): accumulated over row ranges
     double* probs;                   // (dis_count, n_samples, L, L) or nullptr
@@ -46,11 +50,6 @@ struct SampleArgs {
     uint64_t sample_offset, first_disorder;
     unsigned long long* flags;
 };
-
-__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
-    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
-                 : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
-}
 
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
     const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
@@ -67,30 +66,33 @@ __device__ __forceinline__ double quad_sum(double v) {
     return v;
 }
 
-template <int P, bool REALJ, bool F32READ>
-__global__ void __launch_bounds__(SAMPLE_THREADS, 2) sample_rows_kernel(const SampleArgs args) {
+// MT_ = 8-chain M tiles per warp: 2 (128 chains per CTA, the default) or 1 (64 chains per CTA: twice the CTAs of half
+// the size, chosen by the launcher when a 128-chain grid would leave SMs without work -- C2's 100 disorders x 100 samples)
+template <int P, bool REALJ, bool F32READ, int MT_ = SAMPLE_MT>
+__global__ void __launch_bounds__(SAMPLE_THREADS, MT_ == 1 ? 3 : 2) sample_rows_kernel(const SampleArgs args) {
     typedef typename std::conditional<F32READ, float, double>::type TS;   // storage type of the site tensors (TNMC_F32_STORE: float)
     constexpr int KT = P / 4;        // k tiles
     constexpr int NT = P / 4;        // n tiles (2P / 8)
     constexpr int JT = P / 8;        // 8-wide tiles per spin slice
-    constexpr int MT = SAMPLE_MT;
+    constexpr int MT = MT_;
+    constexpr int CHAINS = SAMPLE_WARPS * MT * 8;      // chains per CTA
     constexpr int TSZ = 2 * P * P;
     extern __shared__ __align__(16) double smem[];
     double* sT = smem;                                                    // SAMPLE_STAGES * TSZ
-    uint32_t* sBits = reinterpret_cast<uint32_t*>(smem + SAMPLE_STAGES * TSZ);  // [SAMPLE_CHAINS][W] previous row
+    uint32_t* sBits = reinterpret_cast<uint32_t*>(smem + SAMPLE_STAGES * TSZ);  // [CHAINS][W] previous row
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int g = lane >> 2, q = lane & 3;
     const int L = args.L, W = (L + 31) >> 5;
     // real couplings: (e^{beta J}, e^{-beta J}) of the up bonds of the current row, one entry per column
-    double2* sJ = reinterpret_cast<double2*>(sBits + SAMPLE_CHAINS * W);
+    double2* sJ = reinterpret_cast<double2*>(sBits + CHAINS * W);
     const int dl = blockIdx.y;                       // local disorder index (output indexing)
     const int d = args.dis_begin + dl;               // ctx disorder index (env / J indexing)
     const int tile = blockIdx.x;
     const double beta = args.beta;
     const double eb = exp(beta), emb = exp(-beta);
     const TS* env_d = reinterpret_cast<const TS*>(args.env.base) + (size_t)d * args.env_dis_stride;
-    double* renv = args.renv + ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * (size_t)L * SAMPLE_CHAINS * P;
+    double* renv = args.renv + ((size_t)blockIdx.y * gridDim.x + blockIdx.x) * (size_t)L * CHAINS * P;
 
     // chain handled as M-tile mt, row g of this warp
     int chain_local[MT];      // index within the CTA
@@ -98,12 +100,12 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, 2) sample_rows_kernel(const Sa
 #pragma unroll
     for (int mt = 0; mt < MT; ++mt) {
         chain_local[mt] = (warp * MT + mt) * 8 + g;
-        samp[mt] = (long long)tile * SAMPLE_CHAINS + chain_local[mt];
+        samp[mt] = (long long)tile * CHAINS + chain_local[mt];
     }
     // the "owner" lane of chain (mt = q, g) does that chain's scalar work
     const bool owner = q < MT;
     const int own_local = (warp * MT + (owner ? q : 0)) * 8 + g;
-    const long long own_samp = (long long)tile * SAMPLE_CHAINS + own_local;
+    const long long own_samp = (long long)tile * CHAINS + own_local;
     const bool own_active = owner && own_samp < args.n_samples;
     const size_t own_out = (size_t)dl * args.n_samples + (size_t)(own_active ? own_samp : 0);
     const uint32_t ctr_samp = (uint32_t)(args.sample_offset + (uint64_t)own_samp);
@@ -111,14 +113,21 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, 2) sample_rows_kernel(const Sa
 
     double logq = 0.0;
     if (own_active && args.row_lo > 0) logq = args.logq[own_out];
+    // fused energy / magnetisation (tnmc_sample_fused): the owner lane holds every finished word of the new row and
+    // the word above it, which is all Eq. 1 needs: E = -sum J s s' by XOR + popcount, exactly as energy_kernel
+    const bool fuse = !REALJ && args.E_out != nullptr;
+    int eacc = 0, macc = 0;
+    if (fuse && own_active && args.row_lo > 0) { eacc = args.E_out[own_out]; macc = args.M_out[own_out]; }
+    uint32_t prev_w = 0, prev_rn = 0, prev_rz = 0;   // previous word of the row and its Jr masks (bond across the word boundary)
 
     // previous-row bits of this CTA's chains -> shared (zero for row 0: reading G9, no upper row)
-    for (int t = tid; t < SAMPLE_CHAINS * W; t += SAMPLE_THREADS) {
+    for (int t = tid; t < CHAINS * W; t += SAMPLE_THREADS) {
         const int cl = t / W, w = t % W;
-        const long long s = (long long)tile * SAMPLE_CHAINS + cl;
+        const long long s = (long long)tile * CHAINS + cl;
         uint32_t v = 0;
         if (args.row_lo > 0 && s < args.n_samples)
-            v = args.cfg_bits[(((size_t)dl * args.n_samples + s) * L + (args.row_lo - 1)) * W + w];
+            v = args.cfg_bits != nullptr ? args.cfg_bits[(((size_t)dl * args.n_samples + s) * L + (args.row_lo - 1)) * W + w]
+                                         : args.carry[((size_t)d * args.n_samples_max + s) * W + w];
         sBits[t] = v;
     }
 
@@ -169,7 +178,9 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, 2) sample_rows_kernel(const Sa
                     sJ[c] = make_double2((double)exp(bj), (double)exp(-bj));
                 }
         }
-        uint32_t upw[MT] = {0u, 0u};
+        uint32_t upw[MT];
+#pragma unroll
+        for (int mt = 0; mt < MT; ++mt) upw[mt] = 0u;
         uint32_t jneg = 0, jnz = 0;
         const uint32_t* jd_neg = has_up ? args.J.row(M_JD_NEG, d, r - 1) : nullptr;
         const uint32_t* jd_nz = has_up ? args.J.row(M_JD_NZ, d, r - 1) : nullptr;
@@ -331,7 +342,19 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, 2) sample_rows_kernel(const Sa
                 if (prod < 1e-200) { logq += log(prod); prod = 1.0; }
                 neww |= (uint32_t)a_sel << bit;
                 if (bit == 31 || col == L - 1) {
-                    if (own_active) args.cfg_bits[(own_out * L + r) * W + cur_word] = neww;
+                    if (fuse) {
+                        macc += 2 * __popc(neww) - (bit + 1);
+                        // down bonds (r-1,c)-(r,c): (jneg, jnz) are the masks of Jd row r-1 for this word
+                        if (has_up) eacc -= __popc(jnz) - 2 * __popc((uw ^ neww ^ jneg) & jnz);
+                        // right bonds (r,c)-(r,c+1) inside the word; the bond out of bit 31 waits for the next word
+                        const uint32_t rn = args.J.row(M_JR_NEG, d, r)[cur_word], rz = args.J.row(M_JR_NZ, d, r)[cur_word];
+                        const uint32_t in = rz & 0x7fffffffu;
+                        eacc -= __popc(in) - 2 * __popc(((neww ^ (neww >> 1)) ^ rn) & in);
+                        if (cur_word > 0 && (prev_rz >> 31))
+                            eacc -= 1 - 2 * (int)((((prev_w >> 31) ^ neww) ^ (prev_rn >> 31)) & 1u);
+                        prev_w = neww; prev_rn = rn; prev_rz = rz;
+                    }
+                    if (own_active && args.cfg_bits != nullptr) args.cfg_bits[(own_out * L + r) * W + cur_word] = neww;
                     // sBits of this word is no longer needed by the left sweep: overwrite for the next row
                     sBits[own_local * W + cur_word] = neww;
                 }
@@ -362,7 +385,15 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, 2) sample_rows_kernel(const Sa
         __syncwarp();     // sBits written by owner lanes, read by the whole quad in the next row
     }
     if (own_active) args.logq[own_out] = logq;
+    if (fuse && own_active) { args.E_out[own_out] = eacc; args.M_out[own_out] = macc; }
     cp_async_wait<0>();
+    if (args.cfg_bits == nullptr && args.row_hi < L) {     // configurations not kept: hand the last row to the next row range
+        __syncthreads();
+        for (int t = tid; t < CHAINS * W; t += SAMPLE_THREADS) {
+            const long long s = (long long)tile * CHAINS + t / W;
+            if (s < args.n_samples) args.carry[((size_t)d * args.n_samples_max + s) * W + t % W] = sBits[t];
+        }
+    }
 }
 
 }  // namespace tnmc

@@ -90,13 +90,19 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, 2) sample_rows_tf32_kernel(con
 
     double logq = 0.0;
     if (own_active && args.row_lo > 0) logq = args.logq[own_out];
+    // fused energy / magnetisation (tnmc_sample_fused), as in sample_rows_kernel
+    const bool fuse = !REALJ && args.E_out != nullptr;
+    int eacc = 0, macc = 0;
+    if (fuse && own_active && args.row_lo > 0) { eacc = args.E_out[own_out]; macc = args.M_out[own_out]; }
+    uint32_t prev_w = 0, prev_rn = 0, prev_rz = 0;
 
     for (int t = tid; t < SAMPLE_CHAINS * W; t += SAMPLE_THREADS) {
         const int cl = t / W, w = t % W;
         const long long s = (long long)tile * SAMPLE_CHAINS + cl;
         uint32_t v = 0;
         if (args.row_lo > 0 && s < args.n_samples)
-            v = args.cfg_bits[(((size_t)dl * args.n_samples + s) * L + (args.row_lo - 1)) * W + w];
+            v = args.cfg_bits != nullptr ? args.cfg_bits[(((size_t)dl * args.n_samples + s) * L + (args.row_lo - 1)) * W + w]
+                                         : args.carry[((size_t)d * args.n_samples_max + s) * W + w];
         sBits[t] = v;
     }
 
@@ -312,7 +318,17 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, 2) sample_rows_tf32_kernel(con
                 if (prod < 1e-200) { logq += log(prod); prod = 1.0; }
                 neww |= (uint32_t)a_sel << bit;
                 if (bit == 31 || col == L - 1) {
-                    if (own_active) args.cfg_bits[(own_out * L + r) * W + cur_word] = neww;
+                    if (fuse) {
+                        macc += 2 * __popc(neww) - (bit + 1);
+                        if (has_up) eacc -= __popc(jnz) - 2 * __popc((uw ^ neww ^ jneg) & jnz);
+                        const uint32_t rn = args.J.row(M_JR_NEG, d, r)[cur_word], rz = args.J.row(M_JR_NZ, d, r)[cur_word];
+                        const uint32_t in = rz & 0x7fffffffu;
+                        eacc -= __popc(in) - 2 * __popc(((neww ^ (neww >> 1)) ^ rn) & in);
+                        if (cur_word > 0 && (prev_rz >> 31))
+                            eacc -= 1 - 2 * (int)((((prev_w >> 31) ^ neww) ^ (prev_rn >> 31)) & 1u);
+                        prev_w = neww; prev_rn = rn; prev_rz = rz;
+                    }
+                    if (own_active && args.cfg_bits != nullptr) args.cfg_bits[(own_out * L + r) * W + cur_word] = neww;
                     sBits[own_local * W + cur_word] = neww;
                 }
             }
@@ -342,7 +358,15 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, 2) sample_rows_tf32_kernel(con
         __syncwarp();     // sBits written by owner lanes, read by the whole quad in the next row
     }
     if (own_active) args.logq[own_out] = logq;
+    if (fuse && own_active) { args.E_out[own_out] = eacc; args.M_out[own_out] = macc; }
     cp_async_wait<0>();
+    if (args.cfg_bits == nullptr && args.row_hi < L) {     // configurations not kept: hand the last row to the next row range
+        __syncthreads();
+        for (int t = tid; t < SAMPLE_CHAINS * W; t += SAMPLE_THREADS) {
+            const long long s = (long long)tile * SAMPLE_CHAINS + t / W;
+            if (s < args.n_samples) args.carry[((size_t)d * args.n_samples_max + s) * W + t % W] = sBits[t];
+        }
+    }
 }
 
 }  // namespace tnmc

@@ -36,6 +36,8 @@ def _load():
     lib.tnmc_sample.argtypes = [vp, i32, i32, i32, u64, u64, vp, vp]
     lib.tnmc_sample_ex.restype = i32
     lib.tnmc_sample_ex.argtypes = [vp, i32, i32, i32, u64, u64, vp, vp, vp, vp]
+    lib.tnmc_sample_fused.restype = i32
+    lib.tnmc_sample_fused.argtypes = [vp, i32, i32, i32, u64, u64, vp, vp, vp, vp]
     lib.tnmc_energy.restype = i32
     lib.tnmc_energy.argtypes = [vp, i32, i32, i32, vp, vp]
     lib.tnmc_metropolis.restype = i32
@@ -52,6 +54,8 @@ def _load():
     lib.tnmc_observables.argtypes = [vp, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp]
     lib.tnmc_observables_real.restype = i32
     lib.tnmc_observables_real.argtypes = [vp, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp]
+    lib.tnmc_replica_overlap.restype = i32
+    lib.tnmc_replica_overlap.argtypes = [vp, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.tnmc_observables_static_max.restype = sz
     lib.tnmc_observables_static_max.argtypes = []
     lib.tnmc_observables_static.restype = i32
@@ -172,6 +176,24 @@ class Context:
         _check(st, self.h)
         return cfg_bits, logq
 
+    def tnmc_sample_fused(self, n_samples, seed, sample_offset=0, dis_begin=0, dis_count=None, keep_cfg=True,
+                          cfg_bits=None, logq=None, E=None, M=None):
+        """returns (cfg_bits or None, logq, E, M): E and M come out of the sampling sweep itself"""
+        dis_count = self.n_dis - dis_begin if dis_count is None else dis_count
+        dev = self.device
+        if cfg_bits is None and keep_cfg:
+            cfg_bits = torch.empty((dis_count, n_samples, self.L, self.W), dtype=torch.int32, device=dev)
+        if logq is None:
+            logq = torch.empty((dis_count, n_samples), dtype=torch.float64, device=dev)
+        if E is None:
+            E = torch.empty((dis_count, n_samples), dtype=torch.int32, device=dev)
+        if M is None:
+            M = torch.empty((dis_count, n_samples), dtype=torch.int32, device=dev)
+        _check(lib.tnmc_sample_fused(self.h, dis_begin, dis_count, n_samples, seed, sample_offset,
+                                     _ptr(cfg_bits, torch.int32), _ptr(logq, torch.float64),
+                                     _ptr(E, torch.int32), _ptr(M, torch.int32)), self.h)
+        return cfg_bits, logq, E, M
+
     def tnmc_energy(self, cfg_bits, dis_begin=0, E=None):
         dis_count, n_samples = cfg_bits.shape[0], cfg_bits.shape[1]
         et = torch.float64 if self.real_j else torch.int32
@@ -216,6 +238,21 @@ class Context:
                                     _ptr(accepted, torch.uint8), _ptr(M, torch.int32), _ptr(state[0], et),
                                     _ptr(state[1], torch.int32), _ptr(sums, torch.float64)), self.h)
         return M, state, sums
+
+    def tnmc_replica_overlap(self, cfg_a, accepted_a, cfg_b, accepted_b, state=None, sums=None):
+        """returns (q_steps, (cur_cfg_a, cur_cfg_b), sums) -- sums (dis_count, 3) accumulates q, |q|, q^2 over the steps"""
+        dis_count, n_samples = accepted_a.shape
+        dev = self.device
+        if state is None:
+            state = (torch.zeros((dis_count, self.L, self.W), dtype=torch.int32, device=dev),
+                     torch.zeros((dis_count, self.L, self.W), dtype=torch.int32, device=dev))
+        if sums is None:
+            sums = torch.zeros((dis_count, 3), dtype=torch.float64, device=dev)
+        q = torch.empty((dis_count, n_samples), dtype=torch.int32, device=dev)
+        _check(lib.tnmc_replica_overlap(self.h, dis_count, n_samples, _ptr(cfg_a, torch.int32), _ptr(accepted_a, torch.uint8),
+                                        _ptr(cfg_b, torch.int32), _ptr(accepted_b, torch.uint8), _ptr(state[0], torch.int32),
+                                        _ptr(state[1], torch.int32), _ptr(q, torch.int32), _ptr(sums, torch.float64)), self.h)
+        return q, state, sums
 
     def tnmc_observables_static(self, cfg_bits, E, accepted, state, sums, dis_begin=0):
         """tnmc_observables without any allocation: `state` = (cur_E, cur_M) and `sums` are caller tensors, the

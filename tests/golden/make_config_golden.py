@@ -7,6 +7,7 @@ tests/noise_floor.py; nothing here touches the CUDA path.
     python tests/golden/make_config_golden.py C3      # 2 disorders x 8 samples at 128^2, chi=32, ~1 min
     python tests/golden/make_config_golden.py C4      # 1 disorder x 4 samples at 512^2, ~10 min
     python tests/golden/make_config_golden.py C5      # 1 disorder x 2 samples at 1024^2, ~40 min, ~20 GB of RAM
+                                                      # (OMP_NUM_THREADS=1: the LAPACK calls are 64x128)
 
 Per (beta, disorder) the file holds, from oracle.bmps / oracle.sampler / oracle.exact on the seeded instance
 and the Philox uniforms of reading R (Eq. 1):
@@ -49,8 +50,30 @@ def uniforms(seed, d, n_s, L):
     return philox.spin_uniforms(seed, d, np.arange(n_s)[:, None], sites[None, :]).reshape(n_s, L, L)
 
 
+def build_cache_compact(Jr, Jd, beta, chi, noise_rng=None):
+    """oracle.bmps.build_cache, its loop written out so that every stored row is a compact COPY:
+    the tensors compress() returns are views of the 4x larger LAPACK outputs, which at L = 1024 is 68 GB instead of
+    17 GB.  Same oracle calls in the same order, nothing else.  With noise_rng: tests/noise_floor.perturbed_cache
+    (one rounding error of norm-wise noise per row), likewise compacted."""
+    L = Jr.shape[0]
+    cache = [None] * L
+    logscale = np.zeros(L)
+    mps = bmps.bottom_mps(Jr, beta)
+    cache[L - 1] = mps
+    for row in range(L - 2, -1, -1):
+        mps = bmps.multiply(bmps.row_mpo(Jr, Jd, beta, row), mps)
+        if noise_rng is not None:
+            mps = [A + nf.EPS * np.abs(A).max() * noise_rng.standard_normal(A.shape) for A in mps]
+        ls, mps, _ = bmps.compress(mps, chi)
+        mps = [np.array(A) for A in mps]
+        cache[row] = mps
+        logscale[row] = logscale[row + 1] + ls
+    return cache, logscale
+
+
 def one(L, chi, beta, Jr, Jd, seed, d, n_s, n_p, prob_rows):
-    cache, ls = bmps.build_cache(Jr, Jd, beta, chi)
+    compact = L >= 512
+    cache, ls = build_cache_compact(Jr, Jd, beta, chi) if compact else bmps.build_cache(Jr, Jd, beta, chi)
     lz, sign = bmps.log_z(cache[0], ls[0])
     assert sign == 1.0
     u = uniforms(seed, d, n_s, L)
@@ -58,7 +81,8 @@ def one(L, chi, beta, Jr, Jd, seed, d, n_s, n_p, prob_rows):
     out = dict(logZ=lz, logscale0=ls[0], cfg_bits=pack(cfg), logq=logq, E=exact.energy(cfg, Jr, Jd),
                probs=probs[:n_p][:, prob_rows, :].copy(), min_margin=np.abs(u - probs).min(axis=(1, 2)))
     del cache
-    cache_p, ls_p = nf.perturbed_cache(Jr, Jd, beta, chi)
+    cache_p, ls_p = (build_cache_compact(Jr, Jd, beta, chi, noise_rng=np.random.default_rng(12345)) if compact
+                     else nf.perturbed_cache(Jr, Jd, beta, chi))
     lz_p, _ = bmps.log_z(cache_p[0], ls_p[0])
     fl_p, fl_q = nf.probs_floor(cache_p, Jd, beta, cfg, probs, logq)
     out.update(floor_logZ=abs(lz_p - lz), floor_p=fl_p, floor_logq=fl_q)

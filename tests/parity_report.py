@@ -48,3 +48,35 @@ def check(case, quantity, achieved, nominal, floor=0.0, do_assert=True, **extra)
     if do_assert:
         assert ok, f"{case}: {quantity} deviates by {achieved:.3e} > tol {tol:.3e} ({term}; nominal {nominal:.1e}, floor {floor:.2e})"
     return ok
+
+
+def table(path=None):
+    """markdown summary of a parity_report.jsonl: per (config/beta group, quantity) the worst and median achieved
+    deviation, the tolerance terms that were active and the count of failures.
+        python tests/parity_report.py [gpurun_out/parity_report.jsonl] > profiles/parity_r2.md"""
+    import collections
+    import statistics
+    rows = [json.loads(ln) for ln in open(path or _path())]
+    groups = collections.OrderedDict()
+    for r in rows:
+        case = r["case"]
+        key = (case.split(" d=")[0] + (" " + case.split(" prec=")[1] if " prec=" in case else ""), r["quantity"])
+        groups.setdefault(key, []).append(r)
+    out = ["| case | quantity | n | worst achieved | median | nominal | tolerance terms used (count) | worst tol | failures |",
+           "|---|---|---|---|---|---|---|---|---|"]
+    for (case, qty), rs in groups.items():
+        if qty == "chains":
+            n = sum(r["n"] for r in rs)
+            out.append(f"| {case} | chains bit-identical | {n} | {sum(r['identical'] for r in rs)} identical, "
+                       f"{sum(r['near_threshold'] for r in rs)} near a threshold | | | | | {sum(1 for r in rs if not r['ok'])} |")
+            continue
+        ach = [r["achieved"] for r in rs]
+        terms = collections.Counter(r["term"] for r in rs)
+        out.append(f"| {case} | {qty} | {len(rs)} | {max(ach):.2e} | {statistics.median(ach):.2e} | {rs[0]['nominal']:.0e} | "
+                   + ", ".join(f"{k} ({v})" for k, v in sorted(terms.items())) + f" | {max(r['tol'] for r in rs):.2e} | {sum(1 for r in rs if not r['ok'])} |")
+    return "\n".join(out)
+
+
+if __name__ == "__main__":
+    import sys
+    print(table(sys.argv[1] if len(sys.argv) > 1 else None))

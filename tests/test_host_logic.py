@@ -48,6 +48,13 @@ def test_workspace_bytes_and_argument_errors(lib):
     assert st == 1 and not h.value                                   # TNMC_EINVAL, no context
     lib.tnmc_last_error.restype = ctypes.c_char_p
     assert b"NULL" in lib.tnmc_last_error(None)
+    # the Philox counter word of the disorder index is 32 bits: first_disorder + n_dis beyond 2^32 is refused
+    # (argument check only: the fake pointers are never dereferenced on this path)
+    need = lib.tnmc_workspace_bytes(8, 4, 2, 1, 0, 0)
+    fake = ctypes.c_void_p(1 << 20)
+    st = lib.tnmc_create(ctypes.byref(h), 8, 4, ctypes.c_double(1.0), 2, fake, fake, ctypes.c_uint64((1 << 32) - 1), 1, 0, 0, fake,
+                         ctypes.c_size_t(need), None)
+    assert st == 1 and not h.value and b"2^32" in lib.tnmc_last_error(None)
 
 
 def test_closed_form_bond_dimensions_match_recurrences():

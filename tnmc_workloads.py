@@ -16,6 +16,9 @@ CONFIGS = {
     "C3": dict(L=128, chi=32, betas=(1.0,), n_dis=256, n_samples=256, inst_seed=1003, seed=2003),
     "C4": dict(L=512, chi=32, betas=(1.0,), n_dis=500, n_samples=200, inst_seed=1004, seed=2004),
     "C5": dict(L=1024, chi=32, betas=(1.0,), n_dis=1000, n_samples=1000, inst_seed=1005, seed=2005),
+    # profiling shape: C3's kernels, grid (256 CTAs, two per SM) and per-site work at a quarter of the rows and columns, so that
+    # an `ncu --set full` capture (about 40 replays with device memory saved and restored around each) takes minutes
+    "C3q": dict(L=64, chi=32, betas=(1.0,), n_dis=256, n_samples=256, inst_seed=1003, seed=2003),
     # context only: the paper's own headline setting (chi = 8), in FP64 here
     "C5p": dict(L=1024, chi=8, betas=(1.0,), n_dis=1000, n_samples=1000, inst_seed=1005, seed=2005),
 }
