@@ -43,9 +43,10 @@ WORKLOADS = {
     "C5": ("C5", None, None, 32, "configs[4] 1024x1024 chi=32, 1000 disorders x 1000 samples in 10 chunks of 100 disorders (152 GB of HBM per chunk), checkpoint stride 32", 100),
     "C5c": ("C5", 100, 1000, 32, "configs[4] 1024x1024 chi=32: ONE of the ten 100-disorder chunks of C5 (100 disorders x 1000 samples, 152 GB of HBM), checkpoint stride 32"),
     "C5pf": ("C5p", None, None, 32, "the paper headline setting IN FULL (PAPER.md:286: 1024x1024, chi=8, 1000 disorders x 1000 samples) in 4 chunks of 250 disorders, checkpoint stride 32; run it with --prec f32 for the paper's precision class", 250),
+    "C5c148": ("C5", 148, 1000, 32, "configs[4] 1024x1024 chi=32: a chunk of 148 disorders x 1000 samples (one CTA per SM in the build); fits HBM only with --prec f32s (FP32 stack, FP64 arithmetic), checkpoint stride 32"),
     "C5p": ("C5p", 500, 400, 32, "the paper headline setting (1024x1024, chi=8, PAPER.md:286) in FP64: slice of 500 disorders x 400 samples (one fifth of its 10^6 proposals), checkpoint stride 32"),
 }
-SLICES = ("C4s", "C5s", "C5c", "C5p", "C5pf", "C4", "C5")   # steps of minutes to hours: --warmup is taken as given (0 allowed; said in config)
+SLICES = ("C4s", "C5s", "C5c", "C5c148", "C5p", "C5pf", "C4", "C5")   # steps of minutes to hours: --warmup is taken as given (0 allowed; said in config)
 
 
 def parse():
