@@ -48,7 +48,7 @@ struct BuildCfg {
     static constexpr int LDR = P + 1;         // row length of the carried R_a[x][i]
     static constexpr int LDU = P + 1;         // row length of the carried Pc[z][y]
     static constexpr int TSZ = 2 * P * P;     // doubles per stored site tensor
-    static constexpr int QSZ = LDX * D + D;   // doubles per site of the reflector scratch: image of X + tau
+    static constexpr int QSZ = LDX * D + 2 * D;   // doubles per site of the reflector scratch: image of X + tau + scale
     // shared-memory carve-up (doubles)
     static constexpr int X_OFF = 0;                       // LDX*D : T_0 | T_1 (QR sweep); M, then stage + V_k (SVD sweep)
     static constexpr int Y_OFF = X_OFF + LDX * D;         // D*LDM >= 2*D*LDR, LDX*D : carried R (QR sweep); reflectors, then Jacobi operand
@@ -61,7 +61,7 @@ struct BuildCfg {
     static constexpr int Z_OFF = Y_OFF + Y_SZ;            // D*D   : M before rotation (SVD sweep), P <= 16 only
     static constexpr int U_OFF = Z_OFF + (M0_GLOBAL ? 0 : D * D);   // D*LDU : C_a (QR sweep); carried Pc / M V_k (SVD sweep)
     static constexpr int S_OFF = U_OFF + D * LDU;         // D + 24 + D + 40 : tau / QRCP scratch / sigma / reduction scratch
-    static constexpr int N_DBL = S_OFF + 2 * D + 64 + 48 + 40;
+    static constexpr int N_DBL = S_OFF + 2 * D + 64 + 48 + 40 + D + 8;   // + reflector scales [D] and the QRs' published norms [4]
     static size_t smem_bytes(int L) { return sizeof(double) * N_DBL + sizeof(int) * (L + 2 + 2 * D + 2 + 48); }
 };
 
@@ -80,6 +80,8 @@ __global__ void __launch_bounds__(BuildCfg<P>::NT, BuildCfg<P>::CTAS_PER_SM) bui
     double* sCn = sTau + D;              // [64 + 8] remaining column norms and per-warp partial sums of the QRCP
     double* sSig = sCn + 72;             // [D]  sigma
     double* sRed = sSig + D;             // [40] block reduction scratch
+    double* sScl = sRed + 40;            // [D]  scale of block a's reflectors at a*P (v_j = [1; scale_j x_{i>j}])
+    double* sNrm = sScl + D;             // [4]  squared norm of the next pivot column, two per block QR
     int* sq = reinterpret_cast<int*>(smem + Cfg::N_DBL);   // [L+1] rows q_c of the carried R = left bond of Q_c
     int* spos = sq + args.L + 2;                           // [D] rank / position of each Jacobi row
     int* sperm = spos + D;                                 // [D] step at which each column was the QRCP pivot
@@ -148,7 +150,7 @@ __global__ void __launch_bounds__(BuildCfg<P>::NT, BuildCfg<P>::CTAS_PER_SM) bui
                 break;
             }
             const int p = q < br ? q : br;
-            householder_qr_g<MAXK>(sX + (size_t)half * P * LDX, LDX, q, br, sTau + half * P, gt, HALF, 1 + half);
+            householder_qr_g<MAXK>(sX + (size_t)half * P * LDX, LDX, q, br, sTau + half * P, sScl + half * P, sNrm + 2 * half, gt, HALF, 1 + half);
             __syncthreads();
             // R_new[(a,y)][(rr,k)] = B_r[a][rr] R'_a[y][k] / |R_new|_F;  logscale += log |R_new|_F
             const double jr = args.J.jrv(d, r, c);
@@ -179,6 +181,7 @@ __global__ void __launch_bounds__(BuildCfg<P>::NT, BuildCfg<P>::CTAS_PER_SM) bui
             for (int t = tid; t < 2 * p; t += NT) {
                 const int z = t % p, a = t / p;
                 Qout[LDX * D + a * P + z] = sTau[a * P + z];
+                Qout[LDX * D + D + a * P + z] = sScl[a * P + z];
             }
             __syncthreads();
         }
@@ -222,6 +225,7 @@ __global__ void __launch_bounds__(BuildCfg<P>::NT, BuildCfg<P>::CTAS_PER_SM) bui
                 for (int t = tid; t < 2 * p; t += NT) {
                     const int z = t % p, a = t / p;
                     sTau[a * P + z] = Qin[LDX * D + a * P + z];
+                    sScl[a * P + z] = Qin[LDX * D + D + a * P + z];
                 }
                 for (int t = tid; t < q * nc; t += NT) {
                     const int x = t % q, col = t / q;
@@ -229,7 +233,7 @@ __global__ void __launch_bounds__(BuildCfg<P>::NT, BuildCfg<P>::CTAS_PER_SM) bui
                     sX[(size_t)col * LDX + x] = x < p ? sU[(size_t)(a * p + x) * LDU + y] : 0.0;
                 }
                 __syncthreads();
-                householder_apply_g<MAXK>(sY + (size_t)half * P * LDX, LDX, sTau + half * P, q, p,
+                householder_apply_g<MAXK>(sY + (size_t)half * P * LDX, LDX, sTau + half * P, sScl + half * P, q, p,
                                           sX + (size_t)half * kprev * LDX, LDX, kprev, gt, HALF, 1 + half);
             }
             __syncthreads();

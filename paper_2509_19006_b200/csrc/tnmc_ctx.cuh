@@ -70,7 +70,7 @@ inline bool make_plan(Plan& p, int L, int chi, int n_dis, int n_samples_max, int
         p.n_maps = 1 + p.n_seg;
     }
     p.env_dis_stride = (size_t)p.n_slots * L * p.tsz;
-    p.qsz = (size_t)(2 * p.P + 4) * (2 * p.P) + 2 * p.P;   // BuildCfg<P>::QSZ
+    p.qsz = (size_t)(2 * p.P + 4) * (2 * p.P) + 4 * p.P;   // BuildCfg<P>::QSZ
     p.tiles = (n_samples_max + SAMPLE_CHAINS - 1) / SAMPLE_CHAINS;
     size_t o = 0;
     p.off_masks = o;    o = align_up(o + sizeof(uint32_t) * 4 * (size_t)n_dis * L * p.W);

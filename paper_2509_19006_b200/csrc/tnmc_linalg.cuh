@@ -115,7 +115,7 @@ __device__ __forceinline__ double quad_dot_update_n(const double* __restrict__ v
 // The same update with the UNSCALED pivot column pc (the reflector vector is pc * scale below row j) and the scalars
 // (tau, scale) applied on the fly: w = tau (cj + scale * sum_i pc_i col_i), col_i -= w scale pc_i, row j -> cj - w.
 // Returns the squared norm of the updated rows below j (summed over the quad).
-template <int K>
+template <int K, bool NORM = true>
 __device__ __forceinline__ double quad_pivot_update(const double* __restrict__ pc, double* __restrict__ col,
                                                     int j, int m, int rg, unsigned qmask, double tau, double scale) {
     double x[K], vv[K];
@@ -145,25 +145,27 @@ __device__ __forceinline__ double quad_pivot_update(const double* __restrict__ p
         if (i < m) {
             const double nv = fma(-ws, vv[k], x[k]);
             col[i] = nv;
-            if (k & 1) s1 = fma(nv, nv, s1); else s0 = fma(nv, nv, s0);
+            if (NORM) { if (k & 1) s1 = fma(nv, nv, s1); else s0 = fma(nv, nv, s0); }
         }
     }
     double below2 = s0 + s1;
-    below2 += __shfl_xor_sync(qmask, below2, 1);
-    below2 += __shfl_xor_sync(qmask, below2, 2);
+    if (NORM) {
+        below2 += __shfl_xor_sync(qmask, below2, 1);
+        below2 += __shfl_xor_sync(qmask, below2, 2);
+    }
     if (rg == 0) col[j] = cj - w;
     return below2;
 }
-template <int MAXK>
+template <int MAXK, bool NORM = true>
 __device__ __forceinline__ double quad_pivot_update_n(const double* __restrict__ pc, double* __restrict__ col,
                                                       int j, int m, int rg, unsigned qmask, double tau, double scale) {
     const int rows = m - j - 1;
     if (MAXK >= 4) {
-        if (rows <= MAXK) return quad_pivot_update<(MAXK + 3) / 4>(pc, col, j, m, rg, qmask, tau, scale);
-        if (rows <= 2 * MAXK) return quad_pivot_update<MAXK / 2>(pc, col, j, m, rg, qmask, tau, scale);
-        if (rows <= 3 * MAXK) return quad_pivot_update<(3 * MAXK) / 4>(pc, col, j, m, rg, qmask, tau, scale);
+        if (rows <= MAXK) return quad_pivot_update<(MAXK + 3) / 4, NORM>(pc, col, j, m, rg, qmask, tau, scale);
+        if (rows <= 2 * MAXK) return quad_pivot_update<MAXK / 2, NORM>(pc, col, j, m, rg, qmask, tau, scale);
+        if (rows <= 3 * MAXK) return quad_pivot_update<(3 * MAXK) / 4, NORM>(pc, col, j, m, rg, qmask, tau, scale);
     }
-    return quad_pivot_update<MAXK>(pc, col, j, m, rg, qmask, tau, scale);
+    return quad_pivot_update<MAXK, NORM>(pc, col, j, m, rg, qmask, tau, scale);
 }
 
 // Reflector from alpha = x_j and nrm2 = sum_{i >= j} x_i^2 (the diagonal entry included, so no
@@ -190,63 +192,52 @@ __device__ __forceinline__ void group_bar(int id, int nthreads) {
     asm volatile("bar.sync %0, %1;" :: "r"(id), "r"(nthreads) : "memory");
 }
 
-// Householder QR of the m x n column-major X (leading dim ld) by a group of gn threads (thread gt of
-// the group; gn/4 >= n - 1 quads, m <= 4 * MAXK).  Same algorithm and output as householder_qr.
+// Householder QR of the m x n column-major X (leading dim ld) by a group of gn threads (thread gt of the group;
+// gn/4 >= n - 1 quads, m <= 4 * MAXK).  One barrier per reflector, and nothing serial between barriers: the reflector
+// is kept UNSCALED (v_j = [1; scale_j * x_{i>j}] with x the column as it stands) and its scalars (beta, tau, scale) are
+// derived by every thread from the diagonal entry and the column's remaining squared norm, which the quad that owns
+// column j+1 sums inside its update of step j and publishes before the barrier -- so the rsqrt / reciprocal chain runs
+// beside the loads of the dot product instead of in front of 31 waiting quads, and there is no scaling pass over the
+// column.  (Round 1 built reflector j+1 in one quad between the update and the barrier: 13.7 % of the kernel's warp
+// samples sat at that barrier, profiles/r2c_build32_c3q.md.)
+// On return: R on and above the diagonal of X; below the diagonal of column j the unscaled reflector entries;
+// tau[j], scl[j] its scalars.  nrm: 2 doubles of scratch.  The caller synchronises before reading X.
 template <int MAXK>
-__device__ void householder_qr_g(double* X, int ld, int m, int n, double* tau, int gt, int gn, int bar) {
+__device__ void householder_qr_g(double* X, int ld, int m, int n, double* tau, double* scl, double* nrm, int gt, int gn, int bar) {
     const int kk = m < n ? m : n;
     const int lane = gt & 31;
     const int rg = lane & 3;
     const unsigned qmask = 0xfu << (lane & ~3);
     const int colidx = gt >> 2;
-    if (gt < 32) {     // reflector 0 (first warp of the group)
+    if (gt < 32) {     // squared norm of column 0 (first warp of the group)
         double ss = 0.0;
         for (int i = lane; i < m; i += 32) { const double v = X[i]; ss = fma(v, v, ss); }
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, o);
-        double bet, t, scale;
-        reflector_from_norm(X[0], ss, bet, t, scale);
-        __syncwarp();
-        for (int i = 1 + lane; i < m; i += 32) X[i] *= scale;
-        if (lane == 0) { X[0] = bet; tau[0] = t; }
+        if (lane == 0) nrm[0] = ss;
     }
     group_bar(bar, gn);
     for (int j = 0; j < kk; ++j) {
-        const double* colj = X + (size_t)j * ld;
-        const double t = tau[j];
+        const double* pc = X + (size_t)j * ld;
+        double bet, t, scale;
+        reflector_from_norm(pc[j], nrm[j & 1], bet, t, scale);
         const int jj = j + 1 + colidx;
         if (jj < n) {
             double* col = X + (size_t)jj * ld;
-            double below2;
-            const double w = quad_dot_update_n<MAXK>(colj, col, j + 1, m, rg, qmask, t, col[j], below2);
-            if (rg == 0) col[j] -= w;
-            if (colidx == 0 && j + 1 < kk) {       // build reflector j+1 from the updated column
-                below2 += __shfl_xor_sync(qmask, below2, 1);
-                below2 += __shfl_xor_sync(qmask, below2, 2);
-                __syncwarp(qmask);
-                double bet, t1, scale;
-                reflector_from_norm(col[j + 1], below2, bet, t1, scale);
-                __syncwarp(qmask);
-                {   // scale the new reflector: this quad alone is between the others and the step's barrier, so the
-                    // loads go out together (elementwise, bit-identical to the plain loop)
-                    double tmp[MAXK];
-#pragma unroll
-                    for (int k = 0; k < MAXK; ++k) { const int i = j + 2 + rg + 4 * k; tmp[k] = i < m ? col[i] : 0.0; }
-#pragma unroll
-                    for (int k = 0; k < MAXK; ++k) { const int i = j + 2 + rg + 4 * k; if (i < m) col[i] = tmp[k] * scale; }
-                }
-                if (rg == 0) { col[j + 1] = bet; tau[j + 1] = t1; }
-            }
+            const double below2 = quad_pivot_update_n<MAXK>(pc, col, j, m, rg, qmask, t, scale);
+            if (colidx == 0 && rg == 0) nrm[(j + 1) & 1] = below2;     // rows j+1.. of column j+1: the next reflector's norm
         }
+        if (gt == 0) { tau[j] = t; scl[j] = scale; }
         group_bar(bar, gn);
+        if (gt == 0) X[(size_t)j * ld + j] = bet;     // diagonal of R (column j is read by nobody from here on)
     }
 }
 
-// B <- Q B for the m x nb column-major B (leading dim ldb), Q = H_0 H_1 ... H_{kk-1} given by the
-// reflectors below the diagonal of V (leading dim ldv, unit diagonal implied) and tau, without ever
-// forming Q.  One quad per column of B (gn/4 >= nb); one group barrier per reflector.
+// B <- Q B for the m x nb column-major B (leading dim ldb), Q = H_0 H_1 ... H_{kk-1} given by the unscaled
+// reflectors below the diagonal of V (leading dim ldv; v_j = [1; scl[j] * V_{i>j, j}]) and tau, without ever forming
+// Q.  One quad per column of B (gn/4 >= nb); the columns are independent: no barrier.
 template <int MAXK>
-__device__ void householder_apply_g(const double* V, int ldv, const double* tau, int m, int kk,
+__device__ void householder_apply_g(const double* V, int ldv, const double* tau, const double* scl, int m, int kk,
                                     double* B, int ldb, int nb, int gt, int gn, int bar) {
     const int lane = gt & 31;
     const int rg = lane & 3;
@@ -255,10 +246,7 @@ __device__ void householder_apply_g(const double* V, int ldv, const double* tau,
     if (colidx < nb) {
         double* col = B + (size_t)colidx * ldb;
         for (int j = kk - 1; j >= 0; --j) {
-            double below2;
-            const double w = quad_dot_update_n<MAXK>(V + (size_t)j * ldv, col, j + 1, m, rg, qmask, tau[j], col[j], below2);
-            __syncwarp(qmask);
-            if (rg == 0) col[j] -= w;
+            quad_pivot_update_n<MAXK, false>(V + (size_t)j * ldv, col, j, m, rg, qmask, tau[j], scl[j]);
             __syncwarp(qmask);
         }
     }
@@ -531,20 +519,19 @@ __device__ int jacobi_rows4(double* M, int ld, int nslot, int n, double fro2, do
                 const double g2 = g * g, ab = ao * ap;
                 if (ao > thr2 && ap > thr2 && g2 > rot2 * ab) {
                     big |= g2 > big2 * ab;
-                    // x = the row of smaller index, y = the other: d = |y|^2 - |x|^2, x' = cos x - sin y, y' = cos y + sin x
-                    const bool own_is_x = own < prt;
-                    const double dd = own_is_x ? ap - ao : ao - ap;
+                    // d = |prt|^2 - |own|^2;  own' = cos own + so prt,  prt' = cos prt - so own with so = -sign(d) sin: the
+                    // same rotation whichever member is held (the pair's Jacobi rotation does not depend on the order)
+                    const double dd = ap - ao;
                     const double g24 = 4.0 * g2;
                     const double h2 = fma(dd, dd, g24);
                     const double u = fabs(dd) + h2 * fast_rsqrt1(h2);
                     const double w = fast_rsqrt1(fma(u, u, g24));
                     const double cs = u * w;
-                    double sn = 2.0 * g * w;
-                    if (dd < 0.0) sn = -sn;
-                    const double so = own_is_x ? -sn : sn;         // own' = cos own + so prt,  prt' = cos prt - so own
-                    // norms: |x'|^2 = |x|^2 - t g, |y'|^2 = |y|^2 + t g with t g = sign(d) 2 g^2 / u
+                    const double sn = 2.0 * g * w;
+                    const bool own_grows = dd < 0.0;
+                    const double so = own_grows ? sn : -sn;
+                    // norms: the larger row grows by t g = 2 g^2 / u, the smaller shrinks by it
                     const double qn = 0.5 * g24 * fast_rcp(u);
-                    const bool own_grows = own_is_x == (dd < 0.0);
                     const double apn = own_grows ? ap - qn : ap + qn;
                     ao = own_grows ? ao + qn : ao - qn;
                     if (t8 == 0) y[nslot] = apn;

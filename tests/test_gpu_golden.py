@@ -93,7 +93,7 @@ def _run_case(tn, g, name, bi, ckpt, prec=None, lz_only=False, only=None):
             pr.record(case=case, quantity="chains", n=int(n_s), identical=int(same.sum()), near_threshold=int(near.sum()),
                       ok=bool((same | near).all()))
             ok &= bool((same | near).all())
-            good = same & ~near
+            good = same        # identical spins: everything downstream is comparable, near a threshold or not
             if good.any():
                 o_logq = g["logq"][bi, di]
                 scale = max(1.0, float(np.abs(o_logq).max()))
