@@ -228,7 +228,9 @@ def main_reference(args):
 def bench_config(name, c):
     """the keys both arms print for the same workload"""
     return {"workload": name, "note": c["note"], "L": c["L"], "chi": c["chi"], "betas": list(c["betas"]),
-            "n_dis_per_gpu": c["n_dis"], "n_samples": c["n_samples"], "ckpt_stride": c["ckpt"]}
+            "n_dis_per_gpu": c["n_dis"], "n_samples": c["n_samples"], "ckpt_stride": c["ckpt"],
+            "l2": "GPU arm: flushed (256 MiB memset) before every timed step, in the value loop and in the e2e loop, and the env "
+                  "stack is larger than L2; reference arm: host only"}
 
 
 # ------------------------------------------------------------------------------------------------
@@ -511,13 +513,12 @@ def main_ours(args):
             v_o, dt_o, _, desc_o = oracle_step(c, 15.0)
             cpu = dict(value=v_o, unit="samples/s", kind="oracle", seconds=dt_o, sample=desc_o, **cpu_info())
         cfg_line = bench_config(args.workload, dict(c, n_dis=n_dis_total))
-        cfg_line.update({"couplings": args.couplings, "disorder_chunks": len(chunks), "parallelism": f"dp{world} (disorders sharded, no collective)",
-                         "l2": "flushed (256 MiB memset) before every timed step, in the value loop and in the e2e loop; env stack > L2",
-                         "streams": f"{nb} (one per beta; the launches of each phase run concurrently)"})
+        execution = {"couplings": args.couplings, "disorder_chunks": len(chunks), "parallelism": f"dp{world} (disorders sharded, no collective)",
+                     "streams": f"{nb} (one per beta; the launches of each phase run concurrently)", "prec": args.prec}
         line = {"metric": "accepted samples/s", "value": value, "unit": "samples/s", "n_gpus": world, "steps": args.steps,
                 "warmup": n_warm, "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": {"f64": "f64", "f32": "f64 compression + 3xtf32 sampling (fp32 stack)", "f32s": "f64 arithmetic on an fp32 stack", "tf32": "f64 compression + tf32 sampling (fp32 stack)"}[args.prec], "data": "synthetic",
-                "config": cfg_line,
+                "config": cfg_line, "execution": execution,
                 "chain_sites_per_s": len(betas) * args.steps * n_dis_total * n_s * L * L * world / (ms_total * 1e-3),
                 "flags": dict(flag_tot, note="device counters summed over the timed steps of rank 0 (tnmc_get_flags): near_threshold = draws with |u - p| < 1e-9"),
                 "proposals_per_s": len(betas) * args.steps * n_dis_total * n_s * world / (ms_total * 1e-3),
