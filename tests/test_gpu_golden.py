@@ -77,12 +77,22 @@ def _run_case(tn, g, name, bi, ckpt, prec=None, lz_only=False, only=None):
             bits = bits.cpu().numpy().view(np.uint32)
             logq = logq.cpu().numpy()
             probs = probs.cpu().numpy()[:, :, prob_rows, :]
+        else:
+            # reduced-precision modes: conditionals teacher-forced on the ORACLE's spins (their own spins differ), so that
+            # the comparison is site by site; the mean |dp| is what the mode documents (include/tnmc.h)
+            forced = torch.from_numpy(np.ascontiguousarray(g["cfg_bits"][bi][grp][:, :n_p]).view(np.int32)).to(dev)
+            probs_f = torch.zeros((nd, n_p, L, L), dtype=torch.float64, device=dev)
+            ctx.tnmc_sample(n_p, seed, forced_cfg_bits=forced, probs=probs_f)
+            probs_f = probs_f.cpu().numpy()[:, :, prob_rows, :]
         ctx.close()
         for j, di in enumerate(grp):
             case = f"{name} beta={beta} d={ds[di]}" + (f" prec={prec}" if prec is not None else "")
             lz = float(g["logZ"][bi, di])
             if lz_only:     # reduced-precision modes: north_star's 1e-4 on log Z
                 if not pr.check(case, "logZ_rel", abs(logZ[j] - lz) / abs(lz), 1e-4, do_assert=False):
+                    bad.append(case)
+                dp = np.abs(probs_f[j] - g["probs"][bi, di])
+                if not pr.check(case, "p_mean_abs_forced", dp.mean(), 2e-5, do_assert=False, p_max_abs=float(dp.max())):
                     bad.append(case)
                 continue
             ok = pr.check(case, "logZ_rel", abs(logZ[j] - lz) / abs(lz), 1e-10, float(g["floor_logZ"][bi, di]) / abs(lz), do_assert=False)
