@@ -91,7 +91,7 @@ def test_build_logz_and_states(tn, L, chi, beta, n_dis, seed):
         floor = nf.state_floor(cache, cache_p)
         lz, sign = bmps.log_z(cache[0], ls[0])
         assert sign == 1.0
-        assert abs(logZ[d] - lz) <= max(1e-10 * abs(lz), nf.FLOOR_FACTOR * nf.logz_floor(cache, ls, cache_p, ls_p))
+        assert abs(logZ[d] - lz) <= nf.tol(1e-10 * abs(lz), nf.logz_floor(cache, ls, cache_p, ls_p))
         for r in range(L):
             row, lsr = ctx.tnmc_get_env_row(d, r)
             row = row.numpy()
@@ -104,7 +104,7 @@ def test_build_logz_and_states(tn, L, chi, beta, n_dis, seed):
             v_gpu = bmps.mps_to_vector(mps)
             v_cpu = bmps.mps_to_vector(cache[r])
             scale = np.abs(v_cpu).max()
-            tol = max(1e-10, nf.FLOOR_FACTOR * floor[r])
+            tol = nf.tol(1e-10, floor[r], cap=(L, chi, beta) != (13, 5, 1.3))   # the one deliberately ill-conditioned case
             assert np.abs(v_gpu - v_cpu).max() <= tol * scale
             assert abs(lsr - ls[r]) <= tol * max(1.0, abs(ls[r]))
 
@@ -143,14 +143,14 @@ def test_sample_parity(tn, L, chi, beta, n_dis, n_s, seed):
         o_cfg, o_logq, o_probs = sampler.sample(cache, Jd[d], beta, u)
         cache_p, _ = nf.perturbed_cache(Jr[d], Jd[d], beta, chi)
         fl_p, fl_q = nf.probs_floor(cache_p, Jd[d], beta, o_cfg, o_probs, o_logq)
-        tol_p = max(1e-9, nf.FLOOR_FACTOR * fl_p)
+        tol_p = nf.tol(1e-9, fl_p)
         near = (np.abs(u - o_probs) < tol_p).any(axis=(1, 2))      # chains with a draw too close to call
         n_near += int((np.abs(u - o_probs) < 1e-9).sum())
         ok = ~near
         assert ok.sum() >= 0.9 * n_s
         assert (cfg[d][ok] == o_cfg[ok]).all()
         assert np.abs(probs[d][ok] - o_probs[ok]).max() < tol_p
-        assert np.abs(logq[d][ok] - o_logq[ok]).max() < max(1e-9 * max(1.0, np.abs(o_logq).max()), nf.FLOOR_FACTOR * fl_q)
+        assert np.abs(logq[d][ok] - o_logq[ok]).max() < nf.tol(1e-9 * max(1.0, np.abs(o_logq).max()), fl_q)
         assert (E[d][ok] == exact.energy(o_cfg[ok], Jr[d], Jd[d])).all()
     assert flags["near_threshold"] >= n_near
     assert flags["rho_zero"] == 0 and flags["nonfinite"] == 0

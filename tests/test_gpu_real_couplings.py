@@ -49,21 +49,21 @@ def test_real_couplings_parity(tn, L, chi, beta, n_dis, n_s, k):
         cache_p, ls_p = nf.perturbed_cache(Jr[d], Jd[d], beta, chi)
         lz, sign = bmps.log_z(cache[0], ls[0])
         assert sign == 1.0
-        assert abs(logZ[d] - lz) <= max(1e-10 * abs(lz), nf.FLOOR_FACTOR * nf.logz_floor(cache, ls, cache_p, ls_p))
+        assert abs(logZ[d] - lz) <= nf.tol(1e-10 * abs(lz), nf.logz_floor(cache, ls, cache_p, ls_p))
         u = np.empty((n_s, L, L))
         for r in range(L):
             for c in range(L):
                 u[:, r, c] = philox.spin_uniforms(seed, first + d, np.arange(n_s), r * L + c)
         o_cfg, o_logq, o_probs = sampler.sample(cache, Jd[d], beta, u)
         fl_p, fl_q = nf.probs_floor(cache_p, Jd[d], beta, o_cfg, o_probs, o_logq)
-        tol_p = max(1e-9, nf.FLOOR_FACTOR * fl_p)
+        tol_p = nf.tol(1e-9, fl_p)
         same = (cfg[d] == o_cfg).all(axis=(1, 2))
         near = (np.abs(u - o_probs) < tol_p).any(axis=(1, 2))
         assert (same | near).all()
         ok = same & ~near
         assert ok.sum() >= 0.9 * n_s
         assert np.abs(probs[d].cpu().numpy()[ok] - o_probs[ok]).max() < tol_p
-        assert np.abs(q_h[d][ok] - o_logq[ok]).max() < max(1e-9 * np.abs(o_logq).max(), nf.FLOOR_FACTOR * fl_q)
+        assert np.abs(q_h[d][ok] - o_logq[ok]).max() < nf.tol(1e-9 * np.abs(o_logq).max(), fl_q)
         # energies of the GPU's own configurations (every chain), floating point
         oE = exact.energy_real(cfg[d], Jr[d], Jd[d])
         scale = np.abs(Jr[d]).sum() + np.abs(Jd[d]).sum()
