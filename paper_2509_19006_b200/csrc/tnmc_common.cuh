@@ -25,6 +25,35 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
                  : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
 
+// ---------------------------------------------------------------------------------------------
+// Bulk asynchronous copy global -> shared (TMA engine, `cp.async.bulk`, UBLKCP in SASS) completing on an mbarrier.
+// A stored site tensor is one contiguous, 16-byte aligned block of 0.5 .. 16 KB: the ideal bulk copy -- one instruction by
+// one thread per site instead of one 16-byte cp.async per thread and round.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void mbar_init(uint64_t* bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_init_fence() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;"
+                 :: "r"((unsigned)__cvta_generic_to_shared(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_copy_g2s(void* smem_dst, const void* gmem_src, unsigned bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 :: "r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(gmem_src), "r"(bytes),
+                    "r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity) {
+    asm volatile("{\n"
+                 ".reg .pred p;\n"
+                 "TNMC_MBAR_WAIT:\n"
+                 "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+                 "@p bra TNMC_MBAR_DONE;\n"
+                 "bra TNMC_MBAR_WAIT;\n"
+                 "TNMC_MBAR_DONE:\n"
+                 "}" :: "r"((unsigned)__cvta_generic_to_shared(bar)), "r"(parity) : "memory");
+}
+
 // One warp computes an 8-row strip of C = A B over NT 8-column tiles with DMMA: the A fragment of a k-step is loaded
 // once and used for every column tile.  a_at(g, k), b_at(k, n) return the operand entries (0 outside the matrix),
 // c_out(g, n, v) stores a result.  K is rounded up to a multiple of 4 by the callers' zero padding.

@@ -7,7 +7,7 @@
 // reads it back.  Both sweeps are (chains x chi) x (chi x 2chi) products, run
 // on the FP64 tensor pipe with mma.sync.m8n8k4.f64: 8 chains form the M dimension of one tile,
 // the site tensor (shared by every chain of the disorder) is the B operand, staged through
-// shared memory with a cp.async ring that runs ahead across sweeps and rows.
+// shared memory by a ring of TMA bulk copies (cp.async.bulk + mbarrier) that runs ahead across sweeps and rows.
 //
 // Fragment bookkeeping (see tnmc_common.cuh): with lane = 4*g + q,
 //   A fragment (8x4):  lane holds  V[chain g][k-slot q]          of k-tile kt
@@ -50,15 +50,6 @@ struct SampleArgs {
     uint64_t sample_offset, first_disorder;
     unsigned long long* flags;
 };
-
-__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
-    const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" :: "r"(s), "l"(gmem_src));
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::); }
-template <int N> __device__ __forceinline__ void cp_async_wait() {
-    asm volatile("cp.async.wait_group %0;\n" :: "n"(N));
-}
 
 __device__ __forceinline__ double quad_sum(double v) {
     v += __shfl_xor_sync(0xffffffffu, v, 1);
@@ -137,17 +128,26 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, MT_ == 1 ? 3 : 2) sample_rows_
     (void)n_rows;
     // the tensor stream is addressed with running counters (a 64-bit division per site costs ~60 instructions)
     int pf_r = args.row_lo, pf_t = 0, pf_stage = 0, cur_stage = 0;
+    __shared__ uint64_t s_mbar[SAMPLE_STAGES];       // one mbarrier per stage of the tensor ring
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < SAMPLE_STAGES; ++s) mbar_init(&s_mbar[s], 1);
+        mbar_init_fence();
+    }
+    __syncthreads();
+    unsigned mbar_phase = 0;                          // bit s: parity of the next completion of stage s
     auto issue_prefetch = [&]() {
         if (pf_r < args.row_hi) {
             const int site = pf_t < L - 1 ? (L - 1 - pf_t) : (pf_t - (L - 1));
             const TS* src = env_d + ((size_t)args.slot_of_row[pf_r] * L + site) * TSZ;
             TS* dst = reinterpret_cast<TS*>(sT) + pf_stage * TSZ;
-            constexpr int V = 16 / (int)sizeof(TS);
-            for (int o = tid * V; o < TSZ; o += SAMPLE_THREADS * V) cp_async16(dst + o, src + o);
+            if (tid == 0) {     // one bulk copy of the whole site tensor, completing on the stage's mbarrier
+                mbar_expect_tx(&s_mbar[pf_stage], (unsigned)(TSZ * sizeof(TS)));
+                bulk_copy_g2s(dst, src, (unsigned)(TSZ * sizeof(TS)), &s_mbar[pf_stage]);
+            }
             if (++pf_t == steps_per_row) { pf_t = 0; ++pf_r; }
         }
         if (++pf_stage == SAMPLE_STAGES) pf_stage = 0;
-        cp_async_commit();
     };
     for (int s = 0; s < SAMPLE_STAGES - 1; ++s) issue_prefetch();
 
@@ -186,8 +186,9 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, MT_ == 1 ? 3 : 2) sample_rows_
         const uint32_t* jd_nz = has_up ? args.J.row(M_JD_NZ, d, r - 1) : nullptr;
         int cur_word = -1;
         for (int col = L - 2; col >= 0; --col) {
-            cp_async_wait<SAMPLE_STAGES - 2>();
-            __syncthreads();
+            mbar_wait(&s_mbar[cur_stage], (mbar_phase >> cur_stage) & 1u);   // the tensor of this step has landed
+            mbar_phase ^= 1u << cur_stage;
+            __syncthreads();            // everyone is done with the stage the next copy overwrites
             issue_prefetch();
             const TS* T = reinterpret_cast<const TS*>(sT) + cur_stage * TSZ;   // tensor of site col+1
             if (++cur_stage == SAMPLE_STAGES) cur_stage = 0;
@@ -260,8 +261,9 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, MT_ == 1 ? 3 : 2) sample_rows_
         uint32_t forcedw = 0;
         double prod = 1.0;          // owner lane: running product of chosen probabilities
         for (int col = 0; col < L; ++col) {
-            cp_async_wait<SAMPLE_STAGES - 2>();
-            __syncthreads();
+            mbar_wait(&s_mbar[cur_stage], (mbar_phase >> cur_stage) & 1u);   // the tensor of this step has landed
+            mbar_phase ^= 1u << cur_stage;
+            __syncthreads();            // everyone is done with the stage the next copy overwrites
             issue_prefetch();
             const TS* T = reinterpret_cast<const TS*>(sT) + cur_stage * TSZ;   // tensor of site col
             if (++cur_stage == SAMPLE_STAGES) cur_stage = 0;
@@ -386,7 +388,6 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, MT_ == 1 ? 3 : 2) sample_rows_
     }
     if (own_active) args.logq[own_out] = logq;
     if (fuse && own_active) { args.E_out[own_out] = eacc; args.M_out[own_out] = macc; }
-    cp_async_wait<0>();
     if (args.cfg_bits == nullptr && args.row_hi < L) {     // configurations not kept: hand the last row to the next row range
         __syncthreads();
         for (int t = tid; t < CHAINS * W; t += SAMPLE_THREADS) {

@@ -111,16 +111,26 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, 2) sample_rows_tf32_kernel(con
     (void)n_rows;
     // the tensor stream is addressed with running counters (a 64-bit division per site costs ~60 instructions)
     int pf_r = args.row_lo, pf_t = 0, pf_stage = 0, cur_stage = 0;
+    __shared__ uint64_t s_mbar[SAMPLE_STAGES];       // one mbarrier per stage of the tensor ring
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < SAMPLE_STAGES; ++s) mbar_init(&s_mbar[s], 1);
+        mbar_init_fence();
+    }
+    __syncthreads();
+    unsigned mbar_phase = 0;                          // bit s: parity of the next completion of stage s
     auto issue_prefetch = [&]() {
         if (pf_r < args.row_hi) {
             const int site = pf_t < L - 1 ? (L - 1 - pf_t) : (pf_t - (L - 1));
             const float* src = reinterpret_cast<const float*>(args.env.base) + env_d + ((size_t)args.slot_of_row[pf_r] * L + site) * TSZ;
             float* dst = sT + pf_stage * TSZ;
-            for (int o = tid * 4; o < TSZ; o += SAMPLE_THREADS * 4) cp_async16(dst + o, src + o);
+            if (tid == 0) {     // one bulk copy of the whole site tensor, completing on the stage's mbarrier
+                mbar_expect_tx(&s_mbar[pf_stage], (unsigned)(TSZ * sizeof(float)));
+                bulk_copy_g2s(dst, src, (unsigned)(TSZ * sizeof(float)), &s_mbar[pf_stage]);
+            }
             if (++pf_t == steps_per_row) { pf_t = 0; ++pf_r; }
         }
         if (++pf_stage == SAMPLE_STAGES) pf_stage = 0;
-        cp_async_commit();
     };
     for (int s = 0; s < SAMPLE_STAGES - 1; ++s) issue_prefetch();
 
@@ -156,8 +166,9 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, 2) sample_rows_tf32_kernel(con
         const uint32_t* jd_nz = has_up ? args.J.row(M_JD_NZ, d, r - 1) : nullptr;
         int cur_word = -1;
         for (int col = L - 2; col >= 0; --col) {
-            cp_async_wait<SAMPLE_STAGES - 2>();
-            __syncthreads();
+            mbar_wait(&s_mbar[cur_stage], (mbar_phase >> cur_stage) & 1u);   // the tensor of this step has landed
+            mbar_phase ^= 1u << cur_stage;
+            __syncthreads();            // everyone is done with the stage the next copy overwrites
             issue_prefetch();
             const float* T = sT + cur_stage * TSZ;   // tensor of site col+1
             if (++cur_stage == SAMPLE_STAGES) cur_stage = 0;
@@ -230,8 +241,9 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, 2) sample_rows_tf32_kernel(con
         uint32_t forcedw = 0;
         double prod = 1.0;          // owner lane: running product of chosen probabilities
         for (int col = 0; col < L; ++col) {
-            cp_async_wait<SAMPLE_STAGES - 2>();
-            __syncthreads();
+            mbar_wait(&s_mbar[cur_stage], (mbar_phase >> cur_stage) & 1u);   // the tensor of this step has landed
+            mbar_phase ^= 1u << cur_stage;
+            __syncthreads();            // everyone is done with the stage the next copy overwrites
             issue_prefetch();
             const float* T = sT + cur_stage * TSZ;   // tensor of site col
             if (++cur_stage == SAMPLE_STAGES) cur_stage = 0;
@@ -359,7 +371,6 @@ __global__ void __launch_bounds__(SAMPLE_THREADS, 2) sample_rows_tf32_kernel(con
     }
     if (own_active) args.logq[own_out] = logq;
     if (fuse && own_active) { args.E_out[own_out] = eacc; args.M_out[own_out] = macc; }
-    cp_async_wait<0>();
     if (args.cfg_bits == nullptr && args.row_hi < L) {     // configurations not kept: hand the last row to the next row range
         __syncthreads();
         for (int t = tid; t < SAMPLE_CHAINS * W; t += SAMPLE_THREADS) {

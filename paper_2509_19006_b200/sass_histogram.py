@@ -4,8 +4,8 @@
 
 Runs `cuobjdump -sass` on paper_2509_19006_b200/libtnmc.so and counts, per kernel, the static instructions of the
 opcodes that matter here: DMMA (FP64 tensor pipe, mma.sync.m8n8k4.f64), HMMA (TF32 mma.sync), DFMA/DMUL/DADD (FP64
-ALU), MUFU, LDGSTS (cp.async), LDG/STG/LDS/STS, SHFL, REDUX, BAR, POPC, and the Blackwell-only UTMALDG/UTMASTG (TMA),
-UTC*MMA (tcgen05.mma), LDTM/STTM (TMEM).  Static counts: how often an instruction executes is ncu's business."""
+ALU), MUFU, LDGSTS (cp.async), LDG/STG/LDS/STS, SHFL, REDUX, BAR, POPC, UBLKCP (cp.async.bulk: the TMA engine's bulk copy) and
+SYNCS (mbarrier operations), UTMALDG/UTMASTG (tensor-map TMA), UTC*MMA (tcgen05.mma), LDTM/STTM (TMEM).  Static counts: how often an instruction executes is ncu's business."""
 import collections
 import os
 import re
@@ -14,7 +14,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 OPS = ["DMMA", "HMMA", "DFMA", "DMUL", "DADD", "MUFU", "LDGSTS", "LDG", "STG", "LDS", "STS", "SHFL", "REDUX", "BAR", "POPC",
-       "UTMALDG", "UTMASTG", "UTCHMMA", "UTCQMMA", "LDTM", "STTM"]
+       "UBLKCP", "SYNCS", "UTMALDG", "UTMASTG", "UTCHMMA", "UTCQMMA", "LDTM", "STTM"]
 
 
 def main(show_all):
