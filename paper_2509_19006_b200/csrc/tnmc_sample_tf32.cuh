@@ -53,7 +53,7 @@ __device__ __forceinline__ float quad_sumf(float v) {
 }
 
 template <int P, bool REALJ, bool X3>
-__global__ void __launch_bounds__(SAMPLE_THREADS, 2) sample_rows_tf32_kernel(const SampleArgs args) {
+__global__ void __launch_bounds__(SAMPLE_THREADS, X3 ? 3 : 2) sample_rows_tf32_kernel(const SampleArgs args) {
     constexpr int KT8 = P / 8;       // k tiles (8 bond indices each)
     constexpr int NT = P / 4;        // n tiles (2P / 8)
     constexpr int JT = P / 8;        // 8-wide tiles per spin slice
